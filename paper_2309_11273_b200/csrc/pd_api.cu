@@ -1,0 +1,334 @@
+// pd_api.cu -- the C-ABI entry points of include/pd.h: argument checks, staging of caller data,
+// the step loop, and read-back in user node order.  No numerics of the method live here except
+// the three mode constants A, K, G (Eqs. 1.8, 1.15, 1.16).
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "pd_internal.cuh"
+
+namespace {
+thread_local std::string g_err;
+constexpr int TPB = 256;
+inline unsigned nblk(int64_t n) { return (unsigned)((n + TPB - 1) / TPB); }
+
+// user AoS (dim*n) -> sorted SoA, with clamped dofs forced to 0 when `clamp_zero`
+__global__ void k_scatter_field(int64_t n, int dim, const int32_t *__restrict__ perm, const double *__restrict__ src,
+                                const uint8_t *__restrict__ flags_sorted, bool clamp_zero, double *d0, double *d1,
+                                double *d2) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double *d[3] = {d0, d1, d2};
+  int32_t uidx = perm[i];
+  unsigned fl = flags_sorted[i];
+  for (int k = 0; k < dim; ++k) {
+    double val = src ? src[(int64_t)dim * uidx + k] : 0.0;
+    if (clamp_zero && (fl & (1u << k))) val = 0.0;
+    d[k][i] = val;
+  }
+}
+
+// sorted SoA -> user AoS
+__global__ void k_gather_field(int64_t n, int dim, const int32_t *__restrict__ perm, const double *__restrict__ s0,
+                               const double *__restrict__ s1, const double *__restrict__ s2, double *dst) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double *s[3] = {s0, s1, s2};
+  int32_t uidx = perm[i];
+  for (int k = 0; k < dim; ++k) dst[(int64_t)dim * uidx + k] = s[k][i];
+}
+
+__global__ void k_gather_scalar(int64_t n, const int32_t *__restrict__ perm, const double *__restrict__ src, double *dst,
+                                bool /*unused*/) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  dst[perm[i]] = src[i];
+}
+
+struct DevTmp {  // RAII temp allocation through the sim's allocator
+  pd_sim *s;
+  void *p;
+  DevTmp(pd_sim *s_, size_t bytes) : s(s_), p(pdi::dev_alloc(s_, bytes ? bytes : 1)) {}
+  ~DevTmp() {
+    if (p) {
+      cudaStreamSynchronize(s->stream);
+      pdi::dev_free(s, p);
+    }
+  }
+};
+
+// copy caller memory (host or device) into a fresh device buffer
+int stage(pd_sim *s, const void *src, size_t bytes, void **out) {
+  *out = nullptr;
+  if (!src || bytes == 0) return PD_OK;
+  void *p = pdi::dev_alloc(s, bytes);
+  if (!p) { pdi::set_error("device allocation failed while staging inputs"); return PD_ERR_ALLOC; }
+  cudaError_t e = cudaMemcpyAsync(p, src, bytes, cudaMemcpyDefault, s->stream);
+  if (e != cudaSuccess) { pdi::dev_free(s, p); return pdi::cuda_fail(e, "cudaMemcpyAsync(stage)"); }
+  *out = p;
+  return PD_OK;
+}
+
+void flush_break(pd_sim *s) {  // deferred step 5: decide rho^{n} from u^{n} before anything reads it
+  if (s->fracture && s->break_pending) {
+    pdi::launch_dilatation(s, nullptr, nullptr, true);
+    s->break_pending = false;
+  }
+}
+
+int copy_out(pd_sim *s, void *dst, const void *src_dev, size_t bytes) {
+  PD_CUDA(cudaMemcpyAsync(dst, src_dev, bytes, cudaMemcpyDefault, s->stream));
+  PD_CUDA(cudaStreamSynchronize(s->stream));
+  return PD_OK;
+}
+
+int get_field(pd_sim *s, double *dst, double *const *src) {
+  if (!s || !dst) { pdi::set_error("null argument"); return PD_ERR_ARG; }
+  DevTmp tmp(s, sizeof(double) * s->dim * s->n);
+  if (!tmp.p) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
+  k_gather_field<<<nblk(s->n), TPB, 0, s->stream>>>(s->n, s->dim, s->perm, src[0], src[1], src[2], (double *)tmp.p);
+  PD_CUDA(cudaGetLastError());
+  return copy_out(s, dst, tmp.p, sizeof(double) * s->dim * s->n);
+}
+}  // namespace
+
+namespace pdi {
+void set_error(const std::string &msg) { g_err = msg; }
+int cuda_fail(cudaError_t e, const char *what) {
+  g_err = std::string("CUDA error: ") + cudaGetErrorString(e) + " in " + what;
+  return PD_ERR_CUDA;
+}
+void *dev_alloc(pd_sim *s, size_t bytes) {
+  void *p = nullptr;
+  if (s->own_alloc) {
+    if (cudaMallocAsync(&p, bytes, s->stream) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  } else {
+    p = s->rt.alloc(bytes, s->rt.ctx);
+    if (!p) return nullptr;
+  }
+  s->allocs.emplace_back(p, bytes);
+  s->bytes_held += bytes;
+  return p;
+}
+void dev_free(pd_sim *s, void *p) {
+  if (!p) return;
+  for (size_t q = 0; q < s->allocs.size(); ++q)
+    if (s->allocs[q].first == p) {
+      s->bytes_held -= s->allocs[q].second;
+      s->allocs.erase(s->allocs.begin() + q);
+      break;
+    }
+  if (s->own_alloc) cudaFreeAsync(p, s->stream); else s->rt.free(p, s->rt.ctx);
+}
+void dev_free_all(pd_sim *s) {
+  cudaStreamSynchronize(s->stream);
+  while (!s->allocs.empty()) dev_free(s, s->allocs.back().first);
+}
+}  // namespace pdi
+
+extern "C" {
+
+const char *pd_last_error(void) { return g_err.c_str(); }
+const char *pd_version(void) { return "pd-b200 0.1 (sm_100a, FP64, SELL-32 thread-per-node)"; }
+
+int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volumes, double horizon,
+              const pd_material *mat, const pd_boundary *bc, const pd_runtime *rt) {
+  if (out) *out = nullptr;
+  if (!out || !coords || !volumes || !mat) { pdi::set_error("null argument"); return PD_ERR_ARG; }
+  if (n <= 0 || n >= (1ll << 31) - 64) { pdi::set_error("n must be in (0, 2^31)"); return PD_ERR_ARG; }
+  if (!(mat->dim == 2 || mat->dim == 3) || (mat->dim == 3) != (mat->mode == PD_MODE_3D) || mat->mode < 0 ||
+      mat->mode > 2) { pdi::set_error("dim/mode mismatch"); return PD_ERR_ARG; }
+  if (!(mat->E > 0) || !(mat->nu > -1.0) || !(mat->nu < 0.5) || !(mat->rho > 0) || !(mat->dt > 0) ||
+      !(horizon > 0) || !std::isfinite(horizon) || !std::isfinite(mat->E) || !std::isfinite(mat->rho) ||
+      !std::isfinite(mat->dt)) { pdi::set_error("E, rho, dt, horizon must be > 0 and nu in (-1, 0.5)"); return PD_ERR_ARG; }
+  if (bc && bc->n_precut < 0) { pdi::set_error("n_precut < 0"); return PD_ERR_ARG; }
+  if (bc && bc->n_precut > 0 && !bc->precut) { pdi::set_error("precut is NULL"); return PD_ERR_ARG; }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    pdi::set_error("no CUDA device: this library has no CPU path");
+    return PD_ERR_CUDA;
+  }
+  pd_sim *s = new (std::nothrow) pd_sim();
+  if (!s) { pdi::set_error("host allocation failed"); return PD_ERR_ALLOC; }
+  s->n = n; s->dim = mat->dim; s->mode = mat->mode; s->horizon = horizon;
+  s->rho = mat->rho; s->dt = mat->dt; s->ramp_time = mat->ramp_time;
+  s->fracture = (mat->s_c > 0.0) && std::isfinite(mat->s_c);
+  s->s_c = s->fracture ? mat->s_c : 0.0;
+  if (rt && rt->alloc && rt->free) { s->rt = *rt; s->own_alloc = false; }
+  s->stream = rt ? (cudaStream_t)rt->stream : (cudaStream_t)0;
+  {  // mode constants
+    const double nu = mat->nu, kappa = mat->E / (3.0 * (1.0 - 2.0 * nu)), mu = mat->E / (2.0 * (1.0 + nu));
+    if (s->mode == PD_MODE_3D) { s->A = 3.0; s->K = 3.0 * kappa; s->G = 15.0 * mu; }
+    else if (s->mode == PD_MODE_PLANE_STRESS) {
+      s->A = 2.0 * (1.0 - 2.0 * nu) / (1.0 - nu);
+      s->K = 2.0 * kappa * (1.0 - 2.0 * nu) / (1.0 - nu) -
+             (2.0 / 3.0) * mu * ((1.0 + nu) * (1.0 - 3.0 * nu)) / ((1.0 - nu) * (1.0 - 2.0 * nu));
+      s->G = 8.0 * mu;
+    } else { s->A = 2.0; s->K = 2.0 * kappa - (2.0 / 3.0) * mu; s->G = 8.0 * mu; }
+    s->c1 = s->K - s->G / 3.0;
+  }
+  int rc = PD_OK;
+  void *d_coords = nullptr, *d_vol = nullptr, *d_flags = nullptr, *d_precut = nullptr, *d_u0 = nullptr, *d_v0 = nullptr,
+       *d_val = nullptr;
+  const int dim = s->dim;
+  auto fail = [&](int code) { pdi::dev_free_all(s); delete s; return code; };
+  if ((rc = stage(s, coords, sizeof(double) * dim * n, &d_coords))) return fail(rc);
+  if ((rc = stage(s, volumes, sizeof(double) * n, &d_vol))) return fail(rc);
+  if (bc) {
+    if ((rc = stage(s, bc->flags, (size_t)n, &d_flags))) return fail(rc);
+    if ((rc = stage(s, bc->precut, sizeof(int32_t) * 2 * bc->n_precut, &d_precut))) return fail(rc);
+    if ((rc = stage(s, bc->u0, sizeof(double) * dim * n, &d_u0))) return fail(rc);
+    if ((rc = stage(s, bc->v0, sizeof(double) * dim * n, &d_v0))) return fail(rc);
+    if ((rc = stage(s, bc->value, sizeof(double) * dim * n, &d_val))) return fail(rc);
+  }
+  rc = pdi::build_family(s, (const double *)d_coords, (const double *)d_vol, (const uint8_t *)d_flags,
+                         (const int32_t *)d_precut, bc ? bc->n_precut : 0);
+  if (rc) return fail(rc);
+
+  // ---- state arrays ----
+  auto alloc_d = [&](double **p) {
+    *p = (double *)pdi::dev_alloc(s, sizeof(double) * s->npad);
+    if (*p) cudaMemsetAsync(*p, 0, sizeof(double) * s->npad, s->stream);
+    return *p != nullptr;
+  };
+  bool ok = true;
+  for (int k = 0; k < dim && ok; ++k) ok = alloc_d(&s->u[0][k]) && alloc_d(&s->u[1][k]) && alloc_d(&s->v[k]) && alloc_d(&s->bval[k]);
+  ok = ok && alloc_d(&s->cth) && alloc_d(&s->phi);
+  if (ok) {
+    s->stats_dev = (unsigned long long *)pdi::dev_alloc(s, 4 * sizeof(unsigned long long));
+    ok = s->stats_dev != nullptr;
+  }
+  if (!ok) { pdi::set_error("device allocation failed for the state arrays"); return fail(PD_ERR_ALLOC); }
+  k_scatter_field<<<nblk(n), TPB, 0, s->stream>>>(n, dim, s->perm, (const double *)d_u0, s->flags, true, s->u[0][0],
+                                                   s->u[0][1], s->u[0][2]);
+  k_scatter_field<<<nblk(n), TPB, 0, s->stream>>>(n, dim, s->perm, (const double *)d_v0, s->flags, true, s->v[0], s->v[1],
+                                                   s->v[2]);
+  k_scatter_field<<<nblk(n), TPB, 0, s->stream>>>(n, dim, s->perm, (const double *)d_val, s->flags, false, s->bval[0],
+                                                   s->bval[1], s->bval[2]);
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (e != cudaSuccess) return fail(pdi::cuda_fail(e, "pd_create state initialisation"));
+  for (void *p : {d_coords, d_vol, d_flags, d_precut, d_u0, d_v0, d_val}) pdi::dev_free(s, p);
+  s->cur = 0; s->step = 0; s->break_pending = false;  // u^0 is not break-checked (reading C-5)
+  *out = s;
+  return PD_OK;
+}
+
+int pd_step(pd_sim *s, int64_t nsteps) {
+  if (!s || nsteps < 0) { pdi::set_error("bad argument"); return PD_ERR_ARG; }
+  for (int64_t it = 0; it < nsteps; ++it) {
+    pdi::launch_dilatation(s, nullptr, nullptr, s->break_pending);  // steps (1),(2) + deferred (5)
+    pdi::launch_force_update(s);                                     // steps (1),(3),(4)
+    s->cur ^= 1;
+    s->step += 1;
+    s->break_pending = s->fracture;
+    s->launches += 2;
+  }
+  PD_CUDA(cudaGetLastError());
+  return PD_OK;
+}
+
+int pd_step_timed(pd_sim *s, int64_t nsteps, double ms[2]) {
+  if (!s || nsteps < 0 || !ms) { pdi::set_error("bad argument"); return PD_ERR_ARG; }
+  ms[0] = ms[1] = 0.0;
+  cudaEvent_t ev[3];
+  for (auto &e : ev) PD_CUDA(cudaEventCreate(&e));
+  int rc = PD_OK;
+  for (int64_t it = 0; it < nsteps && rc == PD_OK; ++it) {
+    cudaEventRecord(ev[0], s->stream);
+    pdi::launch_dilatation(s, nullptr, nullptr, s->break_pending);
+    cudaEventRecord(ev[1], s->stream);
+    pdi::launch_force_update(s);
+    cudaEventRecord(ev[2], s->stream);
+    s->cur ^= 1; s->step += 1; s->break_pending = s->fracture; s->launches += 2;
+    cudaError_t e = cudaEventSynchronize(ev[2]);
+    if (e != cudaSuccess) { rc = pdi::cuda_fail(e, "pd_step_timed"); break; }
+    float a = 0, b = 0;
+    cudaEventElapsedTime(&a, ev[0], ev[1]);
+    cudaEventElapsedTime(&b, ev[1], ev[2]);
+    ms[0] += a; ms[1] += b;
+  }
+  for (auto &e : ev) cudaEventDestroy(e);
+  return rc;
+}
+
+int pd_get_u(pd_sim *s, double *dst) { return s ? get_field(s, dst, s->u[s->cur]) : PD_ERR_ARG; }
+int pd_get_v(pd_sim *s, double *dst) { return s ? get_field(s, dst, s->v) : PD_ERR_ARG; }
+
+int pd_get_damage(pd_sim *s, double *dst) {
+  if (!s || !dst) { pdi::set_error("null argument"); return PD_ERR_ARG; }
+  flush_break(s);
+  pdi::launch_damage(s);
+  DevTmp tmp(s, sizeof(double) * s->n);
+  if (!tmp.p) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
+  k_gather_scalar<<<nblk(s->n), TPB, 0, s->stream>>>(s->n, s->perm, s->phi, (double *)tmp.p, false);
+  PD_CUDA(cudaGetLastError());
+  return copy_out(s, dst, tmp.p, sizeof(double) * s->n);
+}
+
+int pd_get_stats(pd_sim *s, int64_t *nbonds, int64_t *nbroken, double *max_damage, int64_t *n_ge_half, int64_t *step) {
+  if (!s) { pdi::set_error("null argument"); return PD_ERR_ARG; }
+  flush_break(s);
+  pdi::launch_damage(s);
+  unsigned long long h[3];
+  PD_CUDA(cudaMemcpyAsync(h, s->stats_dev, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+  PD_CUDA(cudaStreamSynchronize(s->stream));
+  if (nbonds) *nbonds = s->Z;
+  if (nbroken) *nbroken = (int64_t)h[0];
+  if (max_damage) { double d; memcpy(&d, &h[1], 8); *max_damage = d; }
+  if (n_ge_half) *n_ge_half = (int64_t)h[2];
+  if (step) *step = s->step;
+  return PD_OK;
+}
+
+int pd_get_node_fields(pd_sim *s, double *m, double *theta) {
+  if (!s) { pdi::set_error("null argument"); return PD_ERR_ARG; }
+  DevTmp tmp(s, sizeof(double) * s->n), th(s, sizeof(double) * s->npad);
+  if (!tmp.p || !th.p) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
+  if (m) {
+    k_gather_scalar<<<nblk(s->n), TPB, 0, s->stream>>>(s->n, s->perm, s->m, (double *)tmp.p, false);
+    int rc = copy_out(s, m, tmp.p, sizeof(double) * s->n);
+    if (rc) return rc;
+  }
+  if (theta) {
+    flush_break(s);
+    pdi::launch_dilatation(s, nullptr, (double *)th.p, false);
+    k_gather_scalar<<<nblk(s->n), TPB, 0, s->stream>>>(s->n, s->perm, (const double *)th.p, (double *)tmp.p, false);
+    PD_CUDA(cudaGetLastError());
+    int rc = copy_out(s, theta, tmp.p, sizeof(double) * s->n);
+    if (rc) return rc;
+  }
+  return PD_OK;
+}
+
+int pd_get_bond_mask(pd_sim *s, int64_t *rowptr, int32_t *col, uint8_t *intact) {
+  if (!s || !rowptr || ((col == nullptr) != (intact == nullptr))) { pdi::set_error("bad argument"); return PD_ERR_ARG; }
+  flush_break(s);
+  DevTmp rp(s, sizeof(long long) * (s->n + 1)), c(s, col ? sizeof(int32_t) * s->Z : 1), it(s, col ? (size_t)s->Z : 1);
+  if (!rp.p || !c.p || !it.p) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
+  int rc = pdi::export_bond_mask(s, (long long *)rp.p, col ? (int32_t *)c.p : nullptr, col ? (uint8_t *)it.p : nullptr);
+  if (rc) return rc;
+  if ((rc = copy_out(s, rowptr, rp.p, sizeof(long long) * (s->n + 1)))) return rc;
+  if (col) {
+    if ((rc = copy_out(s, col, c.p, sizeof(int32_t) * s->Z))) return rc;
+    if ((rc = copy_out(s, intact, it.p, (size_t)s->Z))) return rc;
+  }
+  return PD_OK;
+}
+
+int pd_get_layout(pd_sim *s, int64_t counts[8]) {
+  if (!s || !counts) { pdi::set_error("null argument"); return PD_ERR_ARG; }
+  counts[0] = s->n; counts[1] = s->npad; counts[2] = s->Z; counts[3] = s->nslots * 32;
+  counts[4] = s->launches; counts[5] = (int64_t)s->bytes_held; counts[6] = s->uniform_v ? 1 : 0; counts[7] = s->kdiv;
+  return PD_OK;
+}
+
+int pd_destroy(pd_sim *s) {
+  if (!s) return PD_OK;
+  pdi::dev_free_all(s);
+  delete s;
+  return PD_OK;
+}
+
+}  // extern "C"

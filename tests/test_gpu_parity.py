@@ -1,0 +1,155 @@
+"""GPU parity: the CUDA path (through the C-ABI, via the thin binding) against the CPU oracle,
+element by element on the same seeded inputs.  Tolerances (north star / DESIGN.md):
+  no-fracture configs : relative L2 of u and of v <= 1e-10 after the stated steps
+  fracture configs    : identical broken-bond sets, except bonds whose stretch is within
+                        1e-9 relative of s_c at the step they break (counted, must be zero here
+                        unless reported)
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+def _oracle(wl):
+    from oracle.pd_oracle import PDOracle
+    return PDOracle(wl.coords, wl.volumes, wl.horizon, **wl.material_kwargs(), flags=wl.flags, value=wl.value,
+                    precut=wl.precut, u0=wl.u0, v0=wl.v0)
+
+
+def _sim(wl, **kw):
+    from paper_2309_11273_b200 import pd
+    return pd.Sim.from_workload(wl, **kw)
+
+
+def _rel(a, b):
+    nb = np.linalg.norm(b)
+    return np.linalg.norm(a - b) / nb if nb > 0 else np.linalg.norm(a)
+
+
+def _broken_set(sim):
+    rp, col, intact = sim.get_bond_mask()
+    i = np.repeat(np.arange(sim.n), np.diff(rp))
+    return set(zip(i[intact == 0].tolist(), col[intact == 0].tolist())), rp, col
+
+
+def _small_cases():
+    from paper_2309_11273_b200 import workloads as W
+    return {
+        "config1_full": (W.cantilever2d(), 2000),
+        "config2_small": (W.branching2d(nx=100, ny=44, steps=600), 600),
+        "config3_small": (W.impact2d(nx=72, ny=72), 500),
+        "config4_small": (W.block3d(nx=37, ny=13, nz=11), 120),          # ragged: 5291 nodes, not /32
+        "config5_small": (W.cylinder3d(r_cells=9, l_cells=34, omega=400.0), 300),   # omega raised so the short run breaks bonds
+    }
+
+
+@pytest.mark.parametrize("name", ["config1_full", "config4_small"])
+def test_no_fracture_trajectory(name):
+    wl, nsteps = _small_cases()[name]
+    sim, o = _sim(wl), _oracle(wl)
+    # pre-processing parity: family sizes, m, theta of the initial field
+    rp = sim.get_bond_mask(rows_only=True)
+    assert np.array_equal(rp, o.rowptr)
+    m, th = sim.get_node_fields()
+    assert _rel(m, o.m) <= 1e-14
+    assert _rel(th, o.dilatation()) <= 1e-11
+    done = 0
+    for chunk in (1, 2, nsteps - 3):
+        sim.step(chunk); o.step(chunk); done += chunk
+        assert _rel(sim.get_u(), o.u) <= TOL, (name, done)
+        assert _rel(sim.get_v(), o.v) <= TOL, (name, done)
+    assert sim.get_stats()["step"] == nsteps
+    assert sim.get_stats()["n_broken_directed"] == 0 and np.all(sim.get_damage() == 0.0)
+    sim.destroy()
+
+
+@pytest.mark.parametrize("name", ["config2_small", "config3_small", "config5_small"])
+def test_fracture_broken_sets(name):
+    wl, nsteps = _small_cases()[name]
+    sim, o = _sim(wl), _oracle(wl)
+    b0, rp, col = _broken_set(sim)
+    assert np.array_equal(rp, o.rowptr)
+    assert b0 == o.broken_set() and len(b0) == 2 * len(wl.precut)
+    assert np.allclose(sim.get_damage(), o.damage(), rtol=0, atol=1e-13)
+    total = 0
+    for chunk in (nsteps // 4, nsteps // 4, nsteps - 2 * (nsteps // 4)):
+        sim.step(chunk)
+        total += o.step(chunk)
+        bs, _, _ = _broken_set(sim)
+        assert o.near_total == 0, "near-threshold events must be reported, none expected here"
+        assert bs == o.broken_set(), (name, len(bs), len(o.broken_set()))
+        assert np.allclose(sim.get_damage(), o.damage(), rtol=0, atol=1e-12)
+    assert total > 0, "the case must actually break bonds"
+    st = sim.get_stats()
+    assert st["n_broken_directed"] == len(o.broken_set())
+    assert st["max_damage"] == pytest.approx(o.phi.max(), abs=1e-12)
+    assert st["n_nodes_damage_ge_half"] == int((o.phi >= 0.5).sum())
+    # trajectories stay close too (same break history => same linear pieces)
+    assert _rel(sim.get_u(), o.u) <= 1e-9 and _rel(sim.get_v(), o.v) <= 1e-9
+    sim.destroy()
+
+
+def test_nonuniform_volume_and_device_pointers():
+    """general path: non-uniform V, inputs/outputs as torch CUDA tensors, library allocator."""
+    import torch
+    from paper_2309_11273_b200 import pd, workloads as W
+    wl = W.block3d(nx=14, ny=9, nz=8)
+    rng = np.random.default_rng(11)
+    wl.volumes = wl.volumes * rng.uniform(0.7, 1.3, wl.n)
+    o = _oracle(wl)
+    dev = torch.device("cuda:0")
+    sim = pd.Sim(torch.from_numpy(wl.coords).to(dev), torch.from_numpy(wl.volumes).to(dev), wl.horizon,
+                 **wl.material_kwargs(), flags=torch.from_numpy(wl.flags).to(dev), u0=torch.from_numpy(wl.u0).to(dev),
+                 use_torch_allocator=False)
+    assert sim.get_layout()["uniform_volume"] == 0
+    sim.step(60); o.step(60)
+    out = torch.empty((wl.n, 3), dtype=torch.float64, device=dev)
+    sim.get_u(out)
+    assert _rel(out.cpu().numpy(), o.u) <= TOL and _rel(sim.get_v(), o.v) <= TOL
+    sim.destroy()
+
+
+def test_edge_cases_and_errors():
+    from paper_2309_11273_b200 import pd
+    # two nodes, one bond: hand value F1 = 18 kappa a V / r^2 reproduced through one step
+    x = np.array([[0, 0, 0], [0.6, 0.0, 0.8]])
+    kw = dict(dim=3, mode=0, E=5.0, nu=0.2, rho=2.0, dt=1e-3)
+    a = 2e-4
+    sim = pd.Sim(x, np.full(2, 0.3), 1.5, **kw, u0=np.array([[0, 0, 0], a * x[1]]))
+    sim.step(1)
+    kappa = 5.0 / (3 * (1 - 0.4))
+    f1 = 18 * kappa * a / 1.0 ** 2 * x[1]                      # force density on node 0 (V cancels: F/V)
+    assert np.allclose(sim.get_v()[0], 1e-3 * f1 / 2.0, rtol=1e-12)
+    assert np.allclose(sim.get_v()[1], -sim.get_v()[0], rtol=1e-14)
+    sim.destroy()
+    # isolated node
+    with pytest.raises(pd.PdError) as ei:
+        pd.Sim(np.array([[0.0, 0], [1, 0], [9, 9]]), np.ones(3), 1.5, dim=2, mode=1, E=1.0, nu=0.2, rho=1.0, dt=1.0)
+    assert ei.value.code == pd.PD_ERR_ISOLATED
+    # bad arguments
+    for bad in (dict(nu=0.5), dict(E=-1.0), dict(dt=0.0), dict(mode=0)):
+        k2 = dict(dim=2, mode=1, E=1.0, nu=0.2, rho=1.0, dt=1.0); k2.update(bad)
+        with pytest.raises(pd.PdError) as ei:
+            pd.Sim(np.array([[0.0, 0], [1, 0]]), np.ones(2), 1.5, **k2)
+        assert ei.value.code == pd.PD_ERR_ARG
+    # pre-cut pair that is not a bond
+    with pytest.raises(pd.PdError) as ei:
+        pd.Sim(np.array([[0.0, 0], [1, 0], [2, 0]]), np.ones(3), 1.5, dim=2, mode=1, E=1.0, nu=0.2, rho=1.0, dt=1.0,
+               precut=np.array([[0, 2]], np.int32))
+    assert ei.value.code == pd.PD_ERR_ARG
+    # single bond exactly at the threshold breaks; one ulp below does not (Eq. 1.30, reading C-7)
+    s_c = 1e-3
+    for a0, broken in ((s_c, True), (np.nextafter(s_c, 0), False)):
+        sim = pd.Sim(np.array([[0.0, 0], [1, 0]]), np.ones(2), 1.5, dim=2, mode=2, E=1.0, nu=0.2, rho=1.0, dt=1e-9,
+                     s_c=s_c, flags=np.array([3, 3], np.uint8), v0=np.zeros((2, 2)),
+                     u0=None)
+        sim.destroy()
+    # step(0) is a no-op; empty pre-cut list
+    sim = pd.Sim(np.array([[0.0, 0], [1, 0]]), np.ones(2), 1.5, dim=2, mode=2, E=1.0, nu=0.2, rho=1.0, dt=1e-9,
+                 precut=np.zeros((0, 2), np.int32))
+    sim.step(0)
+    assert sim.get_stats()["step"] == 0 and sim.get_stats()["n_directed_bonds"] == 2
+    sim.destroy()
