@@ -1,0 +1,280 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement of the OSB-PD explicit step on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config5|config5p|config4|config3|config2|config1]
+    python bench.py --impl reference ...      # the CPU oracle as it stands, on the host cores
+
+A "step" is one pass of the whole hot path (dilatation(+break) kernel, force+update kernel) over
+the workload.  Metric (BASELINE.json): node-steps/s, FP64; bond-updates/s and the HBM roofline of
+the dominant kernel are in the same JSON line.  Default workload = config 5 (3D notched cylinder,
+3.144 M nodes, the config the >=60 %-of-HBM-roofline target is quoted on).
+
+N > 1 (torchrun, one rank per GPU): the path is not sharded ("replicas only"), every
+rank advances an independent replica of the workload; value = N * nodes * K / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "node-steps/s"
+
+
+def make_workload(name):
+    from paper_2309_11273_b200 import workloads as W
+    return W.CONFIGS[name]()
+
+
+def byte_model(n, z, dim, fracture):
+    """Algorithmic bytes per launch (fused minimum B2): per directed bond and pass
+    4 B index + 1/8 B mask; per node 16d+28 B (dilatation pass) and 40d+29 B (force+update pass)."""
+    dil = 4.125 * z + n * (16 * dim + 28 + (8 if fracture else 0))
+    frc = 4.125 * z + n * (40 * dim + 29)
+    return dil, frc
+
+
+class ClockSampler(threading.Thread):
+    """samples nvidia-smi clocks / throttle reasons while the timed region runs"""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag, self.proc = index, [], False, None
+
+    def run(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                self.rows.append((time.time(), [c.strip() for c in line.split(",")]))
+                if self.stop_flag:
+                    break
+        except Exception:
+            pass
+
+    def stop(self):
+        self.stop_flag = True
+        if self.proc:
+            self.proc.terminate()
+
+    def summary(self, t0, t1):
+        rows = [r for t, r in self.rows if t0 <= t <= t1] or [r for _, r in self.rows]
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": len(rows)}
+        try:
+            sm = sorted(float(r[0]) for r in rows)
+            out["sm_mhz"] = sm[len(sm) // 2]
+            out["sm_max_mhz"] = float(rows[0][1])
+            out["power_w_max"] = max(float(r[2]) for r in rows)
+            names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+            out["reasons"] = [nm for k, nm in enumerate(names) if any(r[3 + k].lower().startswith("active") for r in rows)]
+        except Exception:
+            pass
+        return out
+
+
+def oracle_sample(wl_name, steps):
+    """bounded sample of the benchmark workload for the CPU oracle: same cross-section / lattice,
+    material, dt, boundary recipe; fewer nodes and steps (about 10-30 s of CPU work)."""
+    from paper_2309_11273_b200 import workloads as W
+    if wl_name in ("config5", "config5p"):
+        return W.cylinder3d(r_cells=50, l_cells=16), "r=50 cells (full cross-section), L=16 cells = 125 760 nodes", steps
+    if wl_name == "config4":
+        return W.block3d(nx=80, ny=40, nz=40), "80x40x40 = 128 000 nodes", steps
+    return W.CONFIGS[wl_name](), "full workload", steps
+
+
+def time_oracle(wl, steps):
+    from oracle import pd_oracle
+    o = pd_oracle.PDOracle(wl.coords, wl.volumes, wl.horizon, **wl.material_kwargs(), flags=wl.flags, value=wl.value,
+                           precut=wl.precut, u0=wl.u0, v0=wl.v0)
+    t = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t
+    return wl.n * steps / dt, dt, o.Z, pd_oracle.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    wl, desc, _ = oracle_sample(args.workload, args.steps)
+    per_step = max(1, min(args.steps, 50 if wl.dim == 3 else 500))
+    time_oracle(wl, max(1, min(args.warmup, 1)))          # warm-up (page in, build the .so)
+    t0 = time.perf_counter()
+    val, dt, z, cores = time_oracle(wl, per_step)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "node-steps/s", "n_gpus": args.gpus,
+        "steps": per_step, "warmup": 1, "ms_per_step": 1e3 * dt / per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "sample": desc, "nodes": wl.n, "directed_bonds": z},
+        "bond_updates_per_s": z * per_step / dt,
+        "cpu_baseline": {"value": val, "unit": "node-steps/s", "cores": cores, "kind": "oracle",
+                         "sample": f"{desc}, {per_step} steps"},
+        "e2e": {"value": val, "unit": "node-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=300)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config5")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2309_11273_b200 import pd
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    K, Wm = args.steps, max(args.warmup, 3)
+
+    wl = make_workload(args.workload)
+    t0 = time.perf_counter()
+    sim = pd.Sim.from_workload(wl, device=f"cuda:{local}")
+    torch.cuda.synchronize()
+    t_build = time.perf_counter() - t0
+    lay = sim.get_layout()
+    n, z = lay["n"], lay["n_directed_bonds"]
+    fracture = wl.s_c > 0
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps between CUDA events ----
+    sim.step(Wm)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    l0 = sim.get_layout()["step_launches"]
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    tw0 = time.time()
+    ev0.record()
+    sim.step(K)
+    ev1.record()
+    barrier()
+    tw1 = time.time()
+    ms = ev0.elapsed_time(ev1)
+    launches = sim.get_layout()["step_launches"] - l0
+    # ---- per-kernel durations (events around every launch), same state, K more steps ----
+    kd, kf = sim.step_timed(min(K, 100))
+    nk = min(K, 100)
+    sampler.stop()
+    clocks = sampler.summary(tw0, tw1)
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    stats = sim.get_stats()
+    u_max = float(np.abs(sim.get_u()).max()) if rank == 0 else 0.0
+    sim.destroy()
+
+    # ---- end-to-end through the C-ABI with HOST buffers (create + K steps + read-back, all timed) ----
+    e2e = None
+    if not args.no_e2e:
+        host = {k: np.ascontiguousarray(getattr(wl, k)) for k in ("coords", "volumes", "flags", "value", "precut", "u0", "v0")}
+        h2d = sum(a.nbytes for a in host.values())
+        barrier()
+        t0 = time.perf_counter()
+        sim2 = pd.Sim(host["coords"], host["volumes"], wl.horizon, **wl.material_kwargs(), flags=host["flags"],
+                      value=host["value"], precut=host["precut"], u0=host["u0"], v0=host["v0"], device=f"cuda:{local}")
+        sim2.step(K)
+        uo, vo, do = sim2.get_u(), sim2.get_v(), sim2.get_damage()
+        barrier()
+        te = time.perf_counter() - t0
+        d2h = uo.nbytes + vo.nbytes + do.nbytes
+        sim2.destroy()
+        tt = torch.tensor([te], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        te = float(tt.item())
+        e2e = {"value": world * n * K / te, "unit": "node-steps/s", "h2d_bytes_per_step": h2d / K,
+               "d2h_bytes_per_step": d2h / K, "seconds": te,
+               "note": "pd_create from host arrays (family build included) + pd_step(K) + pd_get_u/v/damage to host"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    peak = float(peaks.get("hbm_gbs", 6650.0))
+    peak_kind = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
+    b_dil, b_frc = byte_model(n, z, wl.dim, fracture)
+    t_dil, t_frc = kd / nk * 1e-3, kf / nk * 1e-3
+    dom = ("k_force_update", b_frc, t_frc) if t_frc >= t_dil else ("k_dilatation", b_dil, t_dil)
+    achieved = dom[1] / dom[2] / 1e9
+    step_s = ms * 1e-3 / K
+    line = {
+        "metric": METRIC, "value": world * n * K / (ms * 1e-3), "unit": "node-steps/s", "n_gpus": world, "steps": K,
+        "warmup": Wm, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{args.workload}:{wl.name}", "nodes": n, "directed_bonds": z, "dim": wl.dim,
+                   "fracture": bool(fracture), "horizon_over_dx": 3.015, "l2": "inputs larger than L2 (no flush needed)"
+                   if 4 * z > 2 * 126e6 else "working set fits L2: HBM fraction not meaningful", "parallelism":
+                   "replicas only" if world > 1 else "1 GPU", "build_seconds": t_build},
+        "bond_updates_per_s": world * z * K / (ms * 1e-3),
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": dom[0], "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": None, "peak_kind": peak_kind,
+                     "algorithmic_bytes_per_launch": dom[1], "kernel_ms": dom[2] * 1e3},
+        "kernels": {"k_dilatation": {"ms": t_dil * 1e3, "algorithmic_bytes": b_dil, "GBps": b_dil / t_dil / 1e9},
+                    "k_force_update": {"ms": t_frc * 1e3, "algorithmic_bytes": b_frc, "GBps": b_frc / t_frc / 1e9}},
+        "step_roofline": {"algorithmic_bytes_per_step_B2": b_dil + b_frc, "achieved_GBps": (b_dil + b_frc) / step_s / 1e9,
+                          "frac_of_peak": (b_dil + b_frc) / step_s / 1e9 / peak, "frac_of_8TBps_nominal":
+                          (b_dil + b_frc) / step_s / 8e12},
+        "state": {"broken_directed": stats["n_broken_directed"], "max_damage": stats["max_damage"], "max_abs_u": u_max},
+    }
+    if e2e:
+        line["e2e"] = e2e
+    if not args.no_cpu_baseline:
+        swl, desc, _ = oracle_sample(args.workload, K)
+        osteps = 100 if swl.dim == 3 else 2000
+        val, dt, zz, cores = time_oracle(swl, osteps)
+        line["cpu_baseline"] = {"value": val, "unit": "node-steps/s", "cores": cores, "kind": "oracle",
+                                "sample": f"{desc}, {osteps} steps, {dt:.1f} s"}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
