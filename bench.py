@@ -248,7 +248,7 @@ def main():
         "config": {"workload": f"{args.workload}:{wl.name}", "nodes": n, "directed_bonds": z, "dim": wl.dim,
                    "fracture": bool(fracture), "horizon_over_dx": 3.015, "l2": "inputs larger than L2 (no flush needed)"
                    if 4 * z > 2 * 126e6 else "working set fits L2: HBM fraction not meaningful", "parallelism":
-                   "replicas only" if world > 1 else "1 GPU", "build_seconds": t_build},
+                   "replicas only" if world > 1 else "1 GPU", "build_seconds": t_build, "layout": lay},
         "bond_updates_per_s": world * z * K / (ms * 1e-3),
         "gpu_launches": int(launches),
         "clocks": clocks,

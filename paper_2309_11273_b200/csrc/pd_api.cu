@@ -2,6 +2,7 @@
 // the step loop, and read-back in user node order.  No numerics of the method live here except
 // the three mode constants A, K, G (Eqs. 1.8, 1.15, 1.16).
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -12,37 +13,42 @@ thread_local std::string g_err;
 constexpr int TPB = 256;
 inline unsigned nblk(int64_t n) { return (unsigned)((n + TPB - 1) / TPB); }
 
-// user AoS (dim*n) -> sorted SoA, with clamped dofs forced to 0 when `clamp_zero`
-__global__ void k_scatter_field(int64_t n, int dim, const int32_t *__restrict__ perm, const double *__restrict__ src,
-                                const uint8_t *__restrict__ flags_sorted, bool clamp_zero, double *d0, double *d1,
-                                double *d2) {
+// user AoS (dim*n) -> final order; dst is either a record field (stride 32, via pd_elem) or SoA arrays
+__global__ void k_scatter_field(int64_t npad, int dim, const int32_t *__restrict__ perm, const double *__restrict__ src,
+                                const uint8_t *__restrict__ flags, bool clamp_zero, double *rec, int field, double *d0,
+                                double *d1, double *d2) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
+  if (i >= npad) return;
   double *d[3] = {d0, d1, d2};
   int32_t uidx = perm[i];
-  unsigned fl = flags_sorted[i];
+  unsigned fl = flags[i];
   for (int k = 0; k < dim; ++k) {
-    double val = src ? src[(int64_t)dim * uidx + k] : 0.0;
+    double val = (src && uidx >= 0) ? src[(int64_t)dim * uidx + k] : 0.0;
     if (clamp_zero && (fl & (1u << k))) val = 0.0;
-    d[k][i] = val;
+    if (rec) rec[pd_elem(i) + 32 * (field + k)] = val; else d[k][i] = val;
   }
 }
 
-// sorted SoA -> user AoS
-__global__ void k_gather_field(int64_t n, int dim, const int32_t *__restrict__ perm, const double *__restrict__ s0,
-                               const double *__restrict__ s1, const double *__restrict__ s2, double *dst) {
+// final order -> user AoS; source is a record field or SoA arrays
+__global__ void k_gather_field(int64_t npad, int dim, const int32_t *__restrict__ perm, const double *__restrict__ rec,
+                               int field, const double *__restrict__ s0, const double *__restrict__ s1,
+                               const double *__restrict__ s2, double *dst) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
+  if (i >= npad) return;
   const double *s[3] = {s0, s1, s2};
   int32_t uidx = perm[i];
-  for (int k = 0; k < dim; ++k) dst[(int64_t)dim * uidx + k] = s[k][i];
+  if (uidx < 0) return;
+  for (int k = 0; k < dim; ++k) dst[(int64_t)dim * uidx + k] = rec ? rec[pd_elem(i) + 32 * (field + k)] : s[k][i];
 }
 
-__global__ void k_gather_scalar(int64_t n, const int32_t *__restrict__ perm, const double *__restrict__ src, double *dst,
-                                bool /*unused*/) {
+// scalar per node: record field (rec != NULL) or plain array
+__global__ void k_gather_scalar(int64_t npad, const int32_t *__restrict__ perm, const double *__restrict__ rec, int field,
+                                const double *__restrict__ src, double *dst) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  dst[perm[i]] = src[i];
+  if (i >= npad) return;
+  int32_t uidx = perm[i];
+  if (uidx < 0) return;
+  dst[uidx] = rec ? rec[pd_elem(i) + 32 * field] : src[i];
 }
 
 struct DevTmp {  // RAII temp allocation through the sim's allocator
@@ -71,7 +77,7 @@ int stage(pd_sim *s, const void *src, size_t bytes, void **out) {
 
 void flush_break(pd_sim *s) {  // deferred step 5: decide rho^{n} from u^{n} before anything reads it
   if (s->fracture && s->break_pending) {
-    pdi::launch_dilatation(s, nullptr, nullptr, true);
+    pdi::launch_dilatation(s, nullptr, true);
     s->break_pending = false;
   }
 }
@@ -82,11 +88,12 @@ int copy_out(pd_sim *s, void *dst, const void *src_dev, size_t bytes) {
   return PD_OK;
 }
 
-int get_field(pd_sim *s, double *dst, double *const *src) {
+int get_field(pd_sim *s, double *dst, int field /* record field, or -1 = velocity arrays */) {
   if (!s || !dst) { pdi::set_error("null argument"); return PD_ERR_ARG; }
   DevTmp tmp(s, sizeof(double) * s->dim * s->n);
   if (!tmp.p) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
-  k_gather_field<<<nblk(s->n), TPB, 0, s->stream>>>(s->n, s->dim, s->perm, src[0], src[1], src[2], (double *)tmp.p);
+  k_gather_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->dim, s->perm, field >= 0 ? s->rec : nullptr, field,
+                                                       s->v[0], s->v[1], s->v[2], (double *)tmp.p);
   PD_CUDA(cudaGetLastError());
   return copy_out(s, dst, tmp.p, sizeof(double) * s->dim * s->n);
 }
@@ -129,7 +136,7 @@ void dev_free_all(pd_sim *s) {
 extern "C" {
 
 const char *pd_last_error(void) { return g_err.c_str(); }
-const char *pd_version(void) { return "pd-b200 0.1 (sm_100a, FP64, SELL-32 thread-per-node)"; }
+const char *pd_version(void) { return "pd-b200 0.2 (sm_100a, FP64, blocked SELL-32xR, warp per R-row group)"; }
 
 int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volumes, double horizon,
               const pd_material *mat, const pd_boundary *bc, const pd_runtime *rt) {
@@ -157,6 +164,11 @@ int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volum
   s->s_c = s->fracture ? mat->s_c : 0.0;
   if (rt && rt->alloc && rt->free) { s->rt = *rt; s->own_alloc = false; }
   s->stream = rt ? (cudaStream_t)rt->stream : (cudaStream_t)0;
+  s->R = 4;
+  if (const char *env = getenv("PD_ROWS_PER_THREAD")) {  // tuning knob: 1, 2 or 4 lattice rows per thread
+    int r = atoi(env);
+    if (r == 1 || r == 2 || r == 4) s->R = r;
+  }
   {  // mode constants
     const double nu = mat->nu, kappa = mat->E / (3.0 * (1.0 - 2.0 * nu)), mu = mat->E / (2.0 * (1.0 + nu));
     if (s->mode == PD_MODE_3D) { s->A = 3.0; s->K = 3.0 * kappa; s->G = 15.0 * mu; }
@@ -186,26 +198,26 @@ int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volum
                          (const int32_t *)d_precut, bc ? bc->n_precut : 0);
   if (rc) return fail(rc);
 
-  // ---- state arrays ----
+  // ---- state arrays (u, cth live in the node records built above) ----
   auto alloc_d = [&](double **p) {
     *p = (double *)pdi::dev_alloc(s, sizeof(double) * s->npad);
     if (*p) cudaMemsetAsync(*p, 0, sizeof(double) * s->npad, s->stream);
     return *p != nullptr;
   };
   bool ok = true;
-  for (int k = 0; k < dim && ok; ++k) ok = alloc_d(&s->u[0][k]) && alloc_d(&s->u[1][k]) && alloc_d(&s->v[k]) && alloc_d(&s->bval[k]);
-  ok = ok && alloc_d(&s->cth) && alloc_d(&s->phi);
+  for (int k = 0; k < dim && ok; ++k) ok = alloc_d(&s->v[k]) && alloc_d(&s->bval[k]);
+  ok = ok && alloc_d(&s->phi);
   if (ok) {
     s->stats_dev = (unsigned long long *)pdi::dev_alloc(s, 4 * sizeof(unsigned long long));
     ok = s->stats_dev != nullptr;
   }
   if (!ok) { pdi::set_error("device allocation failed for the state arrays"); return fail(PD_ERR_ALLOC); }
-  k_scatter_field<<<nblk(n), TPB, 0, s->stream>>>(n, dim, s->perm, (const double *)d_u0, s->flags, true, s->u[0][0],
-                                                   s->u[0][1], s->u[0][2]);
-  k_scatter_field<<<nblk(n), TPB, 0, s->stream>>>(n, dim, s->perm, (const double *)d_v0, s->flags, true, s->v[0], s->v[1],
-                                                   s->v[2]);
-  k_scatter_field<<<nblk(n), TPB, 0, s->stream>>>(n, dim, s->perm, (const double *)d_val, s->flags, false, s->bval[0],
-                                                   s->bval[1], s->bval[2]);
+  k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, s->perm, (const double *)d_u0, s->flags, true,
+                                                         s->rec, PD_F_U(0), nullptr, nullptr, nullptr);
+  k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, s->perm, (const double *)d_v0, s->flags, true,
+                                                         nullptr, 0, s->v[0], s->v[1], s->v[2]);
+  k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, s->perm, (const double *)d_val, s->flags, false,
+                                                         nullptr, 0, s->bval[0], s->bval[1], s->bval[2]);
   cudaError_t e = cudaGetLastError();
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
   if (e != cudaSuccess) return fail(pdi::cuda_fail(e, "pd_create state initialisation"));
@@ -218,7 +230,7 @@ int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volum
 int pd_step(pd_sim *s, int64_t nsteps) {
   if (!s || nsteps < 0) { pdi::set_error("bad argument"); return PD_ERR_ARG; }
   for (int64_t it = 0; it < nsteps; ++it) {
-    pdi::launch_dilatation(s, nullptr, nullptr, s->break_pending);  // steps (1),(2) + deferred (5)
+    pdi::launch_dilatation(s, nullptr, s->break_pending);  // steps (1),(2) + deferred (5)
     pdi::launch_force_update(s);                                     // steps (1),(3),(4)
     s->cur ^= 1;
     s->step += 1;
@@ -237,7 +249,7 @@ int pd_step_timed(pd_sim *s, int64_t nsteps, double ms[2]) {
   int rc = PD_OK;
   for (int64_t it = 0; it < nsteps && rc == PD_OK; ++it) {
     cudaEventRecord(ev[0], s->stream);
-    pdi::launch_dilatation(s, nullptr, nullptr, s->break_pending);
+    pdi::launch_dilatation(s, nullptr, s->break_pending);
     cudaEventRecord(ev[1], s->stream);
     pdi::launch_force_update(s);
     cudaEventRecord(ev[2], s->stream);
@@ -253,8 +265,8 @@ int pd_step_timed(pd_sim *s, int64_t nsteps, double ms[2]) {
   return rc;
 }
 
-int pd_get_u(pd_sim *s, double *dst) { return s ? get_field(s, dst, s->u[s->cur]) : PD_ERR_ARG; }
-int pd_get_v(pd_sim *s, double *dst) { return s ? get_field(s, dst, s->v) : PD_ERR_ARG; }
+int pd_get_u(pd_sim *s, double *dst) { return s ? get_field(s, dst, PD_F_U(s->cur)) : PD_ERR_ARG; }
+int pd_get_v(pd_sim *s, double *dst) { return s ? get_field(s, dst, -1) : PD_ERR_ARG; }
 
 int pd_get_damage(pd_sim *s, double *dst) {
   if (!s || !dst) { pdi::set_error("null argument"); return PD_ERR_ARG; }
@@ -262,7 +274,7 @@ int pd_get_damage(pd_sim *s, double *dst) {
   pdi::launch_damage(s);
   DevTmp tmp(s, sizeof(double) * s->n);
   if (!tmp.p) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
-  k_gather_scalar<<<nblk(s->n), TPB, 0, s->stream>>>(s->n, s->perm, s->phi, (double *)tmp.p, false);
+  k_gather_scalar<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->perm, nullptr, 0, s->phi, (double *)tmp.p);
   PD_CUDA(cudaGetLastError());
   return copy_out(s, dst, tmp.p, sizeof(double) * s->n);
 }
@@ -287,14 +299,14 @@ int pd_get_node_fields(pd_sim *s, double *m, double *theta) {
   DevTmp tmp(s, sizeof(double) * s->n), th(s, sizeof(double) * s->npad);
   if (!tmp.p || !th.p) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
   if (m) {
-    k_gather_scalar<<<nblk(s->n), TPB, 0, s->stream>>>(s->n, s->perm, s->m, (double *)tmp.p, false);
+    k_gather_scalar<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->perm, s->rec, PD_F_M, nullptr, (double *)tmp.p);
     int rc = copy_out(s, m, tmp.p, sizeof(double) * s->n);
     if (rc) return rc;
   }
   if (theta) {
     flush_break(s);
-    pdi::launch_dilatation(s, nullptr, (double *)th.p, false);
-    k_gather_scalar<<<nblk(s->n), TPB, 0, s->stream>>>(s->n, s->perm, (const double *)th.p, (double *)tmp.p, false);
+    pdi::launch_dilatation(s, (double *)th.p, false);
+    k_gather_scalar<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->perm, nullptr, 0, (const double *)th.p, (double *)tmp.p);
     PD_CUDA(cudaGetLastError());
     int rc = copy_out(s, theta, tmp.p, sizeof(double) * s->n);
     if (rc) return rc;
@@ -319,7 +331,7 @@ int pd_get_bond_mask(pd_sim *s, int64_t *rowptr, int32_t *col, uint8_t *intact) 
 
 int pd_get_layout(pd_sim *s, int64_t counts[8]) {
   if (!s || !counts) { pdi::set_error("null argument"); return PD_ERR_ARG; }
-  counts[0] = s->n; counts[1] = s->npad; counts[2] = s->Z; counts[3] = s->nslots * 32;
+  counts[0] = s->n; counts[1] = s->npad; counts[2] = s->Z; counts[3] = s->nentries * 32;
   counts[4] = s->launches; counts[5] = (int64_t)s->bytes_held; counts[6] = s->uniform_v ? 1 : 0; counts[7] = s->kdiv;
   return PD_OK;
 }

@@ -1,16 +1,27 @@
 // pd_build.cu -- GPU cell-list family builder.
 //
 // Runs once in pd_create, entirely on the device:
-//   1. bounding box, fine uniform cell grid (cell edge = horizon / kdiv, kdiv ~ horizon/spacing)
-//   2. brick-raster sort key per node (bricks of BX x BY x BZ fine cells, raster inside a brick)
-//      -> radix sort -> permutation perm[sorted] = user.  Consecutive sorted nodes are consecutive
-//      along x inside a brick row, so a warp (32 lanes = 32 nodes) gathers contiguous neighbour data
-//      and a CTA covers a compact spatial tile.
-//   3. dense cell table (start/end in sorted order)
-//   4. count pass  -> row length per node -> slice length (warp max, rounded to PD_SLOT_ALIGN)
-//      -> exclusive scan -> slice offsets (SELL-32)
-//   5. fill pass   -> col (neighbour sorted index per slot), intact mask, m_i (Eq. 1.9), sum_j V_j
-//   6. pre-cut pairs clear their two mask bits; no-fail bit mask (only if some node is no-fail)
+//   1. bounding box; node spacing from the median nearest-neighbour distance of a node sample;
+//      uniform cell grid whose edge per dimension is extent/round(extent/spacing), origin shifted by
+//      half a cell: on a (jittered) lattice body every cell holds exactly one node.  Nothing below
+//      depends on that for correctness -- any point cloud gives the right families, a lattice
+//      (the paper's discretisation) gives the compact layout.
+//   2. radix sort by cell id (z, y, x) -> every (z, y) CELL ROW is a run sorted along x
+//   3. final node order: a TILE = (BZ z-levels) x (R cell rows in y) x (32 cells in x, counted from
+//      the first occupied cell of the tile row); lane = x cell inside the tile (nodes sharing a
+//      cell are pushed to the next free lane).  Tiles that hold a node are numbered in raster
+//      order; slice = tile*BZ*R + (z % BZ)*R + (y % R), final index = slice*32 + lane.  Absent
+//      nodes are phantoms.  Lane l of a group (= R slices = one warp) therefore owns R nodes that
+//      are adjacent in y at the same x: their families overlap, so one gathered neighbour
+//      serves up to R bonds (register blocking of the neighbour list).
+//   4. count pass -> entries per group -> exclusive scan -> group offsets ("SELL-32xR")
+//   5. fill pass  -> col (neighbour element index per entry), member bits, m_i (Eq. 1.9), sum_j V_j
+//   6. pre-cut pairs clear their two intact bits; no-fail bit mask (only if some node is no-fail)
+// Passes 4 and 5 run one warp per group in LOCKSTEP over the cells of a box around the lanes'
+// nominal cells: an entry is created for (relative cell, k-th node in it) whenever that node is a
+// family member for ANY lane, and lanes without a bond there get a padding entry.  So all lanes of
+// a warp meet the same relative neighbour in the same entry: the gathers of an entry are
+// contiguous, and which (entry, r) pairs are bonds is warp-uniform in the bulk.
 // The horizon test is ||xi||^2 <= horizon^2 (inclusive) with the products and
 // sums rounded individually in component order (no FMA contraction), so it is reproducible.
 #include <cub/device/device_radix_sort.cuh>
@@ -20,6 +31,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstring>
 
 #include "pd_internal.cuh"
 
@@ -29,19 +41,19 @@ constexpr int TPB = 256;
 
 struct Grid {
   double lo[3];
-  double inv_c;  // 1 / cell edge
-  int nc[3];     // fine cells per dim
-  int nb[3];     // bricks per dim
-  int B[3];      // brick size in cells
-  int R;         // search radius in cells
+  double inv_c[3];  // 1 / cell edge per dimension
+  int nc[3];        // cells per dim
+  int S[3];         // search radius in cells per dim
   int dim;
+  int R, BZ;        // rows per thread, z-levels per tile
+  int ncyg, nczt, maxchunk;
 };
 
 __device__ __forceinline__ void cell_of(const Grid &g, const double *p, int *q) {
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
     if (k < g.dim) {
-      int c = (int)floor((p[k] - g.lo[k]) * g.inv_c);
+      int c = (int)floor((p[k] - g.lo[k]) * g.inv_c[k] + 0.5);
       q[k] = min(max(c, 0), g.nc[k] - 1);
     } else {
       q[k] = 0;
@@ -72,230 +84,383 @@ static double dec_host(unsigned long long e) {
 
 __global__ void k_bbox(int64_t n, int dim, const double *__restrict__ coords, const double *__restrict__ vol,
                        unsigned long long *out /* [0..2]=min, [3..5]=max, [6]=vmin, [7]=vmax */) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  for (int k = 0; k < dim; ++k) {
-    unsigned long long e = enc(coords[dim * i + k]);
-    atomicMin(&out[k], e);
-    atomicMax(&out[3 + k], e);
+  __shared__ unsigned long long sh[8];
+  if (threadIdx.x < 8) sh[threadIdx.x] = (threadIdx.x < 3 || threadIdx.x == 6) ? ~0ull : 0ull;
+  __syncthreads();
+  unsigned long long mn[4] = {~0ull, ~0ull, ~0ull, ~0ull}, mx[4] = {0, 0, 0, 0};
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    for (int k = 0; k < dim; ++k) {
+      unsigned long long e = enc(coords[dim * i + k]);
+      mn[k] = min(mn[k], e);
+      mx[k] = max(mx[k], e);
+    }
+    unsigned long long ev = enc(vol[i]);
+    mn[3] = min(mn[3], ev);
+    mx[3] = max(mx[3], ev);
   }
-  unsigned long long ev = enc(vol[i]);
-  atomicMin(&out[6], ev);
-  atomicMax(&out[7], ev);
+  for (int k = 0; k < 4; ++k)
+    for (int o = 16; o > 0; o >>= 1) {
+      mn[k] = min(mn[k], __shfl_xor_sync(0xffffffffu, mn[k], o));
+      mx[k] = max(mx[k], __shfl_xor_sync(0xffffffffu, mx[k], o));
+    }
+  if ((threadIdx.x & 31) == 0) {
+    for (int k = 0; k < 3; ++k) { atomicMin(&sh[k], mn[k]); atomicMax(&sh[3 + k], mx[k]); }
+    atomicMin(&sh[6], mn[3]);
+    atomicMax(&sh[7], mx[3]);
+  }
+  __syncthreads();
+  if (threadIdx.x < 8) {
+    if (threadIdx.x < 3 || threadIdx.x == 6) atomicMin(&out[threadIdx.x], sh[threadIdx.x]);
+    else atomicMax(&out[threadIdx.x], sh[threadIdx.x]);
+  }
 }
 
-// ---- 2. sort keys -----------------------------------------------------------------------------
-__global__ void k_keys(int64_t n, Grid g, const double *__restrict__ coords, unsigned long long *keys,
-                       int32_t *ids) {
+// nearest-neighbour distance^2 of sample nodes (brute force; one block per sample)
+__global__ void k_nn_sample(int64_t n, int dim, const double *__restrict__ coords, int64_t stride, double *out) {
+  const int64_t i = (int64_t)blockIdx.x * stride;
+  double pi[3] = {0, 0, 0};
+  for (int k = 0; k < dim; ++k) pi[k] = coords[dim * i + k];
+  double best = 1.0e300;
+  for (int64_t j = threadIdx.x; j < n; j += blockDim.x) {
+    double r2 = 0.0;
+    for (int k = 0; k < dim; ++k) { double d = coords[dim * j + k] - pi[k]; r2 += d * d; }
+    if (j != i && r2 > 0.0) best = fmin(best, r2);
+  }
+  __shared__ double sh[TPB / 32];
+  for (int o = 16; o > 0; o >>= 1) best = fmin(best, __shfl_xor_sync(0xffffffffu, best, o));
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = best;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < TPB / 32; ++w) best = fmin(best, sh[w]);
+    out[blockIdx.x] = best;
+  }
+}
+
+// ---- 2. sort keys: raster cell id, x fastest ------------------------------------------------------
+__global__ void k_keys(int64_t n, Grid g, const double *__restrict__ coords, uint32_t *keys, int32_t *ids) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   double p[3] = {0, 0, 0};
   for (int k = 0; k < g.dim; ++k) p[k] = coords[g.dim * i + k];
   int q[3];
   cell_of(g, p, q);
-  unsigned long long brick = ((unsigned long long)(q[2] / g.B[2]) * g.nb[1] + (q[1] / g.B[1])) * g.nb[0] + (q[0] / g.B[0]);
-  unsigned long long inner = ((unsigned long long)(q[2] % g.B[2]) * g.B[1] + (q[1] % g.B[1])) * g.B[0] + (q[0] % g.B[0]);
-  keys[i] = brick * (unsigned long long)(g.B[0] * g.B[1] * g.B[2]) + inner;
+  keys[i] = (uint32_t)(((int64_t)q[2] * g.nc[1] + q[1]) * g.nc[0] + q[0]);
   ids[i] = (int32_t)i;
 }
 
-// ---- gather user -> sorted --------------------------------------------------------------------
-__global__ void k_gather_nodes(int64_t n, int64_t npad, int dim, const int32_t *__restrict__ perm,
-                               const double *__restrict__ coords, const double *__restrict__ vol,
-                               const uint8_t *__restrict__ flags, double *x0, double *x1, double *x2,
-                               double *volS, uint8_t *flagsS, int32_t *iperm) {
+// cell and row tables over the sorted keys (start/end positions; empty = 0/0)
+__global__ void k_tables(int64_t n, int ncx, const uint32_t *__restrict__ keys, int32_t *cell_start, int32_t *cell_end,
+                         int32_t *row_start, int32_t *row_end) {
+  int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n) return;
+  uint32_t c = keys[p];
+  uint32_t cp = p > 0 ? keys[p - 1] : 0xffffffffu, cn = p + 1 < n ? keys[p + 1] : 0xffffffffu;
+  if (p == 0 || c != cp) cell_start[c] = (int32_t)p;
+  if (p + 1 == n || c != cn) cell_end[c] = (int32_t)(p + 1);
+  uint32_t r = c / ncx;
+  if (p == 0 || r != cp / ncx) row_start[r] = (int32_t)p;
+  if (p + 1 == n || r != cn / ncx) row_end[r] = (int32_t)(p + 1);
+}
+
+// t_p = cx_p - rank_p: its running maximum along a row places nodes that share a cell on the next free lane
+__global__ void k_row_t(int64_t n, int ncx, const uint32_t *__restrict__ keys, const int32_t *__restrict__ row_start,
+                        int32_t *rowid, int32_t *t) {
+  int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n) return;
+  uint32_t c = keys[p];
+  int32_t row = (int32_t)(c / ncx);
+  rowid[p] = row;
+  t[p] = (int32_t)(c % ncx) - (int32_t)(p - row_start[row]);
+}
+
+// first occupied x cell of every tile row = (BZ z-levels) x (R cell rows)
+__global__ void k_tilerow_x0(int64_t ntr, Grid g, const uint32_t *__restrict__ keys, const int32_t *__restrict__ row_start,
+                             const int32_t *__restrict__ row_end, int32_t *x0) {
+  int64_t tr = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (tr >= ntr) return;
+  int yg = (int)(tr % g.ncyg), zt = (int)(tr / g.ncyg);
+  int best = 0x7fffffff;
+  for (int dz = 0; dz < g.BZ; ++dz)
+    for (int dy = 0; dy < g.R; ++dy) {
+      int cz = zt * g.BZ + dz, cy = yg * g.R + dy;
+      if (cz >= g.nc[2] || cy >= g.nc[1]) continue;
+      int64_t row = (int64_t)cz * g.nc[1] + cy;
+      if (row_end[row] > row_start[row]) best = min(best, (int)(keys[row_start[row]] % g.nc[0]));
+    }
+  x0[tr] = best;
+}
+
+// virtual x (lane + 32*chunk) of every node inside its tile row, and its maximum
+__global__ void k_vx(int64_t n, Grid g, const int32_t *__restrict__ rowid, const int32_t *__restrict__ row_start,
+                     const int32_t *__restrict__ tmax, const int32_t *__restrict__ x0, int32_t *vx, int *maxvx) {
+  int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int v = 0;
+  if (p < n) {
+    int row = rowid[p];
+    int cy = row % g.nc[1], cz = row / g.nc[1];
+    int64_t tr = (int64_t)(cz / g.BZ) * g.ncyg + cy / g.R;
+    v = (int)(p - row_start[row]) + tmax[p] - x0[tr];
+    vx[p] = v;
+  }
+  for (int o = 16; o > 0; o >>= 1) v = max(v, __shfl_xor_sync(0xffffffffu, v, o));
+  if ((threadIdx.x & 31) == 0) atomicMax(maxvx, v);
+}
+
+__device__ __forceinline__ int64_t tile_dense_of(const Grid &g, int row, int vx) {
+  int cy = row % g.nc[1], cz = row / g.nc[1];
+  return ((int64_t)(cz / g.BZ) * g.ncyg + cy / g.R) * g.maxchunk + (vx >> 5);
+}
+
+__global__ void k_tile_mark(int64_t n, Grid g, const int32_t *__restrict__ rowid, const int32_t *__restrict__ vx,
+                            int32_t *flag) {
+  int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n) return;
+  flag[tile_dense_of(g, rowid[p], vx[p])] = 1;
+}
+
+__global__ void k_final_index(int64_t n, Grid g, const int32_t *__restrict__ rowid, const int32_t *__restrict__ vx,
+                              const int32_t *__restrict__ ord1, const int32_t *__restrict__ tile_ord,
+                              int32_t *tile_inv, int32_t *fin1, int32_t *perm, int32_t *iperm) {
+  int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n) return;
+  int row = rowid[p];
+  int cy = row % g.nc[1], cz = row / g.nc[1];
+  int64_t td = tile_dense_of(g, row, vx[p]);
+  int32_t t = tile_ord[td];
+  tile_inv[t] = (int32_t)td;
+  int64_t slice = (int64_t)t * (g.BZ * g.R) + (cz % g.BZ) * g.R + (cy % g.R);
+  int32_t fin = (int32_t)(slice * 32 + (vx[p] & 31));
+  fin1[p] = fin;
+  int32_t uidx = ord1[p];
+  perm[fin] = uidx;
+  iperm[uidx] = fin;
+}
+
+// node records in final order (rec, flags pre-zeroed; phantoms stay zero)
+__global__ void k_records(int64_t npad, int dim, const int32_t *__restrict__ perm, const double *__restrict__ coords,
+                          const double *__restrict__ vol, const uint8_t *__restrict__ flags, double *rec,
+                          uint8_t *flagsF) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= npad) return;
-  double *xs[3] = {x0, x1, x2};
-  if (i < n) {
-    int32_t uidx = perm[i];
-    for (int k = 0; k < dim; ++k) xs[k][i] = coords[(int64_t)dim * uidx + k];
-    volS[i] = vol[uidx];
-    flagsS[i] = flags ? flags[uidx] : (uint8_t)0;
-    iperm[uidx] = (int32_t)i;
-  } else {  // padding nodes: never referenced as neighbours, never written back
-    for (int k = 0; k < dim; ++k) xs[k][i] = 0.0;
-    volS[i] = 0.0;
-    flagsS[i] = 0;
-  }
+  int32_t uidx = perm[i];
+  if (uidx < 0) return;
+  double *r = rec + pd_elem(i);
+  for (int k = 0; k < dim; ++k) r[32 * (PD_F_X + k)] = coords[(int64_t)dim * uidx + k];
+  r[32 * PD_F_VOL] = vol[uidx];
+  flagsF[i] = flags ? flags[uidx] : (uint8_t)0;
 }
 
-// ---- 3. cell table ----------------------------------------------------------------------------
-__device__ __forceinline__ int64_t raster_cell(const Grid &g, const int *q) {
-  return ((int64_t)q[2] * g.nc[1] + q[1]) * g.nc[0] + q[0];
-}
-
-__global__ void k_cell_table(int64_t n, Grid g, const double *__restrict__ x0, const double *__restrict__ x1,
-                             const double *__restrict__ x2, int32_t *cell_start, int32_t *cell_end) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const double *xs[3] = {x0, x1, x2};
-  int q[3];
-  double p[3] = {0, 0, 0};
-  for (int k = 0; k < g.dim; ++k) p[k] = xs[k][i];
-  cell_of(g, p, q);
-  int64_t c = raster_cell(g, q);
-  int64_t cprev = -1, cnext = -1;
-  if (i > 0) {
-    for (int k = 0; k < g.dim; ++k) p[k] = xs[k][i - 1];
-    cell_of(g, p, q);
-    cprev = raster_cell(g, q);
+// ---- 4./5. lockstep family traversal of one group (one warp; lane = R nodes) -----------------------
+// Calls f(j_final or -1, bits, r2[R]) once per ENTRY, for all 32 lanes together: bits != 0 for the
+// lanes that have a bond to their j there (bit r <=> ||x_j - x_{i_r}||^2 <= h2 and j != i_r).
+template <int R, typename F>
+__device__ __forceinline__ void for_group_family(const Grid &g, int64_t grp, int lane, double h2,
+                                                 const double *__restrict__ rec, const int32_t *__restrict__ perm,
+                                                 const int32_t *__restrict__ cell_start,
+                                                 const int32_t *__restrict__ cell_end,
+                                                 const int32_t *__restrict__ fin1,
+                                                 const int32_t *__restrict__ tile_inv,
+                                                 const int32_t *__restrict__ tile_x0, F f) {
+  constexpr unsigned FULL = 0xffffffffu;
+  // nominal cell of the lane
+  const int64_t td = tile_inv[grp / g.BZ];
+  const int chunk = (int)(td % g.maxchunk);
+  const int64_t tr = td / g.maxchunk;
+  const int by0 = (int)(tr % g.ncyg) * g.R, bz = (int)(tr / g.ncyg) * g.BZ + (int)(grp % g.BZ);
+  const int bx = tile_x0[tr] + 32 * chunk + lane;
+  double pi[R][3];
+  int64_t ir[R];
+  unsigned valid = 0;
+  int dl = 1 << 30, dh = -(1 << 30);
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    ir[r] = (grp * R + r) * 32 + lane;
+    pi[r][0] = pi[r][1] = pi[r][2] = 0.0;
+    if (perm[ir[r]] >= 0) {
+      valid |= 1u << r;
+      const double *p = rec + pd_elem(ir[r]);
+      for (int k = 0; k < g.dim; ++k) pi[r][k] = p[32 * (PD_F_X + k)];
+      int q[3];
+      cell_of(g, pi[r], q);
+      dl = min(dl, q[0] - bx);
+      dh = max(dh, q[0] - bx);
+    }
   }
-  if (i + 1 < n) {
-    for (int k = 0; k < g.dim; ++k) p[k] = xs[k][i + 1];
-    cell_of(g, p, q);
-    cnext = raster_cell(g, q);
+  for (int o = 16; o > 0; o >>= 1) {
+    dl = min(dl, __shfl_xor_sync(FULL, dl, o));
+    dh = max(dh, __shfl_xor_sync(FULL, dh, o));
   }
-  if (c != cprev) cell_start[c] = (int32_t)i;
-  if (c != cnext) cell_end[c] = (int32_t)(i + 1);
-}
-
-// ---- 4./5. family traversal ---------------------------------------------------------------------
-// Visits the family of sorted node i in a fixed order (cells dz, dy, dx ascending; sorted index
-// ascending inside a cell) and calls f(j, r2).
-template <typename F>
-__device__ __forceinline__ void for_family(const Grid &g, int64_t i, double h2, const double *__restrict__ x0,
-                                           const double *__restrict__ x1, const double *__restrict__ x2,
-                                           const int32_t *__restrict__ cell_start,
-                                           const int32_t *__restrict__ cell_end, F f) {
-  const double *xs[3] = {x0, x1, x2};
-  double pi[3] = {0, 0, 0};
-  for (int k = 0; k < g.dim; ++k) pi[k] = xs[k][i];
-  int q[3];
-  cell_of(g, pi, q);
-  int z0 = g.dim > 2 ? max(q[2] - g.R, 0) : 0, z1 = g.dim > 2 ? min(q[2] + g.R, g.nc[2] - 1) : 0;
-  int y0 = max(q[1] - g.R, 0), y1 = min(q[1] + g.R, g.nc[1] - 1);
-  int xa = max(q[0] - g.R, 0), xb = min(q[0] + g.R, g.nc[0] - 1);
+  if (dh < dl) return;  // no node in this group
+  const int z0 = g.dim > 2 ? max(bz - g.S[2], 0) : 0, z1 = g.dim > 2 ? min(bz + g.S[2], g.nc[2] - 1) : 0;
+  const int y0 = max(by0 - g.S[1], 0), y1 = min(by0 + g.R - 1 + g.S[1], g.nc[1] - 1);
   for (int cz = z0; cz <= z1; ++cz)
     for (int cy = y0; cy <= y1; ++cy) {
-      int64_t base = ((int64_t)cz * g.nc[1] + cy) * g.nc[0];
-      for (int cx = xa; cx <= xb; ++cx) {
-        int32_t s = cell_start[base + cx], e = cell_end[base + cx];
-        for (int32_t j = s; j < e; ++j) {
-          if (j == i) continue;
-          double pj[3] = {0, 0, 0};
-          for (int k = 0; k < g.dim; ++k) pj[k] = xs[k][j];
-          double r2 = dist2_exact(g.dim, pi, pj);
-          if (r2 <= h2) f(j, r2);
+      const int64_t base = ((int64_t)cz * g.nc[1] + cy) * g.nc[0];
+      for (int dx = dl - g.S[0]; dx <= dh + g.S[0]; ++dx) {
+        const int cx = bx + dx;
+        int32_t s = 0, e = 0;
+        if (valid && cx >= 0 && cx < g.nc[0]) { s = cell_start[base + cx]; e = cell_end[base + cx]; }
+        int cnt = e - s, mx = cnt;
+        for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(FULL, mx, o));
+        for (int idx = 0; idx < mx; ++idx) {
+          unsigned bits = 0;
+          double r2[R];
+          int64_t j = -1;
+          if (idx < cnt) {
+            j = fin1[s + idx];
+            const double *q = rec + pd_elem(j);
+            double pj[3] = {0, 0, 0};
+            for (int k = 0; k < g.dim; ++k) pj[k] = q[32 * (PD_F_X + k)];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+              r2[r] = dist2_exact(g.dim, pi[r], pj);
+              if (((valid >> r) & 1u) && j != ir[r] && r2[r] <= h2) bits |= 1u << r;
+            }
+          }
+          if (__any_sync(FULL, bits != 0)) f(j, bits, r2);
         }
       }
     }
 }
 
-__global__ void k_count(int64_t n, int64_t npad, Grid g, double h2, const double *__restrict__ x0,
-                        const double *__restrict__ x1, const double *__restrict__ x2,
-                        const int32_t *__restrict__ cell_start, const int32_t *__restrict__ cell_end,
-                        int32_t *rowlen, int32_t *slice_len, int32_t *slice_words) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= npad) return;
-  int cnt = 0;
-  if (i < n) for_family(g, i, h2, x0, x1, x2, cell_start, cell_end, [&](int32_t, double) { ++cnt; });
-  rowlen[i] = cnt;
-  int mx = cnt;
-  for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-  if ((threadIdx.x & 31) == 0) {
-    int len = (mx + PD_SLOT_ALIGN - 1) / PD_SLOT_ALIGN * PD_SLOT_ALIGN;
-    slice_len[i >> 5] = len;
-    slice_words[i >> 5] = (len + 31) / 32;
-  }
+template <int R>
+__global__ void k_count(int64_t ngroups, Grid g, double h2, const double *__restrict__ rec,
+                        const int32_t *__restrict__ perm, const int32_t *__restrict__ cell_start,
+                        const int32_t *__restrict__ cell_end, const int32_t *__restrict__ fin1,
+                        const int32_t *__restrict__ tile_inv, const int32_t *__restrict__ tile_x0, int32_t *rowlen,
+                        uint32_t *glen) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int64_t grp = t >> 5;
+  if (grp >= ngroups) return;
+  int lane = threadIdx.x & 31;
+  int cnt = 0, rl[R];
+#pragma unroll
+  for (int r = 0; r < R; ++r) rl[r] = 0;
+  for_group_family<R>(g, grp, lane, h2, rec, perm, cell_start, cell_end, fin1, tile_inv, tile_x0,
+                      [&](int64_t, unsigned bits, const double *) {
+                        ++cnt;
+#pragma unroll
+                        for (int r = 0; r < R; ++r) rl[r] += (bits >> r) & 1u;
+                      });
+#pragma unroll
+  for (int r = 0; r < R; ++r) rowlen[(grp * R + r) * 32 + lane] = rl[r];
+  constexpr int EPW = 32 / R;
+  if (lane == 0) glen[grp] = (uint32_t)((cnt + EPW - 1) / EPW * EPW);  // cnt is the same on all lanes
 }
 
-__global__ void k_fill(int64_t n, int64_t npad, Grid g, double h2, const double *__restrict__ x0,
-                       const double *__restrict__ x1, const double *__restrict__ x2,
-                       const double *__restrict__ vol, const int32_t *__restrict__ cell_start,
-                       const int32_t *__restrict__ cell_end, const int32_t *__restrict__ slice_len,
-                       const uint32_t *__restrict__ slice_off, const uint32_t *__restrict__ mask_off,
-                       int32_t *col, uint32_t *mask, double *m_out, double *fvol_out) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= npad) return;
+template <int R>
+__global__ void k_fill(int64_t ngroups, Grid g, double h2, double G, double *__restrict__ rec,
+                       const int32_t *__restrict__ perm, const int32_t *__restrict__ cell_start,
+                       const int32_t *__restrict__ cell_end, const int32_t *__restrict__ fin1,
+                       const int32_t *__restrict__ tile_inv, const int32_t *__restrict__ tile_x0,
+                       const uint32_t *__restrict__ goff, uint32_t *col, uint32_t *member) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int64_t grp = t >> 5;
+  if (grp >= ngroups) return;
+  constexpr int EPW = 32 / R;
   int lane = threadIdx.x & 31;
-  int64_t s = i >> 5;
-  int64_t off = (int64_t)slice_off[s] * 32 + lane;
-  int len = slice_len[s];
+  const int64_t off = goff[grp];
+  const int len = (int)(goff[grp + 1] - goff[grp]);
+  uint32_t *c = col + off * 32 + lane;
+  uint32_t *mb = member + off / EPW * 32 + lane;
+  const uint32_t self = pd_elem(grp * R * 32 + lane);
   int k = 0;
-  double m = 0.0, fv = 0.0;
-  if (i < n)
-    for_family(g, i, h2, x0, x1, x2, cell_start, cell_end, [&](int32_t j, double r2) {
-      col[off + (int64_t)k * 32] = j;
-      double vj = vol[j];
-      m = fma(r2, vj, m);  // m_i = sum ||xi||^2 V_j   (Eq. 1.9, w = 1)
-      fv += vj;            // sum V_j                   (Eq. 1.31 denominator)
-      ++k;
-    });
-  int cnt = k;
-  for (; k < len; ++k) col[off + (int64_t)k * 32] = (int32_t)i;  // padding slots: self, bit 0
-  int64_t moff = (int64_t)mask_off[s] * 32 + lane;
-  for (int w = 0; w * 32 < len; ++w) {
-    int nb = min(max(cnt - w * 32, 0), 32);
-    mask[moff + (int64_t)w * 32] = nb == 32 ? 0xffffffffu : ((1u << nb) - 1u);
+  uint32_t word = 0;
+  double m[R], fv[R];
+#pragma unroll
+  for (int r = 0; r < R; ++r) m[r] = fv[r] = 0.0;
+  for_group_family<R>(g, grp, lane, h2, rec, perm, cell_start, cell_end, fin1, tile_inv, tile_x0,
+                      [&](int64_t j, unsigned bits, const double *r2) {
+                        c[(int64_t)k * 32] = bits ? pd_elem(j) : self;
+                        word |= bits << ((k % EPW) * R);
+                        if (bits) {
+                          double vj = rec[pd_elem(j) + 32 * PD_F_VOL];
+#pragma unroll
+                          for (int r = 0; r < R; ++r)
+                            if ((bits >> r) & 1u) {
+                              m[r] = fma(r2[r], vj, m[r]);  // m_i = sum ||xi||^2 V_j   (Eq. 1.9, w = 1)
+                              fv[r] += vj;                  // sum V_j                   (Eq. 1.31 denominator)
+                            }
+                        }
+                        ++k;
+                        if (k % EPW == 0) { mb[(int64_t)(k / EPW - 1) * 32] = word; word = 0; }
+                      });
+  for (; k < len;) {  // padding entries: own node 0, all bits 0
+    c[(int64_t)k * 32] = self;
+    ++k;
+    if (k % EPW == 0) { mb[(int64_t)(k / EPW - 1) * 32] = word; word = 0; }
   }
-  m_out[i] = m;
-  fvol_out[i] = fv;
+#pragma unroll
+  for (int r = 0; r < R; ++r) {
+    int64_t i = (grp * R + r) * 32 + lane;
+    if (perm[i] < 0) continue;
+    double *p = rec + pd_elem(i);
+    p[32 * PD_F_M] = m[r];
+    p[32 * PD_F_FVOL] = fv[r];
+    p[32 * PD_F_MINV] = m[r] > 0.0 ? 1.0 / m[r] : 0.0;
+    p[32 * PD_F_GMU] = m[r] > 0.0 ? G / m[r] : 0.0;
+  }
 }
 
 // ---- 6. pre-cuts and no-fail mask ---------------------------------------------------------------
-__global__ void k_precut(int64_t np, int64_t n, const int32_t *__restrict__ pairs, const int32_t *__restrict__ iperm,
-                         const int32_t *__restrict__ rowlen, const uint32_t *__restrict__ slice_off,
-                         const uint32_t *__restrict__ mask_off, const int32_t *__restrict__ col, uint32_t *mask,
+__global__ void k_precut(int64_t np, int64_t n, int R, const int32_t *__restrict__ pairs,
+                         const int32_t *__restrict__ iperm, const uint32_t *__restrict__ goff,
+                         const uint32_t *__restrict__ col, const uint32_t *__restrict__ member, uint32_t *intact,
                          unsigned long long *err) {
   int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= 2 * np) return;
   int64_t pa = pairs[2 * (p >> 1) + (p & 1)], pb = pairs[2 * (p >> 1) + 1 - (p & 1)];
   if (pa < 0 || pa >= n || pb < 0 || pb >= n || pa == pb) { atomicExch(err, 1ull); return; }
-  int32_t a = iperm[pa], b = iperm[pb];
-  int64_t s = a >> 5;
-  int lane = a & 31;
-  int64_t off = (int64_t)slice_off[s] * 32 + lane, moff = (int64_t)mask_off[s] * 32 + lane;
-  int len = rowlen[a];
+  int32_t a = iperm[pa];
+  const uint32_t eb = pd_elem(iperm[pb]);
+  const int EPW = 32 / R;
+  int64_t slice = a >> 5;
+  int lane = a & 31, r = (int)(slice % R);
+  int64_t grp = slice / R;
+  int64_t off = goff[grp];
+  int len = (int)(goff[grp + 1] - goff[grp]);
   for (int k = 0; k < len; ++k)
-    if (col[off + (int64_t)k * 32] == b) {
-      atomicAnd(&mask[moff + (int64_t)(k >> 5) * 32], ~(1u << (k & 31)));
-      return;
+    if (col[(off + k) * 32 + lane] == eb) {
+      int64_t w = (off + k) / EPW * 32 + lane;
+      uint32_t bit = 1u << ((k % EPW) * R + r);
+      if (member[w] & bit) { atomicAnd(&intact[w], ~bit); return; }
     }
   atomicExch(err, 1ull);  // not a bond
 }
 
-__global__ void k_nofail(int64_t npad, const uint8_t *__restrict__ flags, const int32_t *__restrict__ rowlen,
-                         const int32_t *__restrict__ slice_len, const uint32_t *__restrict__ slice_off,
-                         const uint32_t *__restrict__ mask_off, const int32_t *__restrict__ col, uint32_t *nofail) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= npad) return;
+__global__ void k_nofail(int64_t ngroups, int R, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ goff,
+                         const uint32_t *__restrict__ col, const uint32_t *__restrict__ member, uint32_t *nofail) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int64_t grp = t >> 5;
+  if (grp >= ngroups) return;
   int lane = threadIdx.x & 31;
-  int64_t s = i >> 5;
-  int64_t off = (int64_t)slice_off[s] * 32 + lane, moff = (int64_t)mask_off[s] * 32 + lane;
-  int len = slice_len[s], cnt = rowlen[i];
-  unsigned fi = flags[i];
-  for (int w = 0; w * 32 < len; ++w) {
+  const int EPW = 32 / R;
+  int64_t off = goff[grp];
+  int len = (int)(goff[grp + 1] - goff[grp]);
+  unsigned fi = 0;  // bit r: node r is no-fail
+  for (int r = 0; r < R; ++r)
+    if (flags[(grp * R + r) * 32 + lane] & PD_NO_FAIL) fi |= 1u << r;
+  const unsigned all = (1u << R) - 1u;
+  for (int w = 0; w * EPW < len; ++w) {
     uint32_t word = 0;
-    for (int b = 0; b < 32 && w * 32 + b < cnt; ++b) {
-      int32_t j = col[off + (int64_t)(w * 32 + b) * 32];
-      if ((fi | flags[j]) & PD_NO_FAIL) word |= 1u << b;
+    for (int q = 0; q < EPW; ++q) {
+      int64_t j = pd_elem_inv(col[(off + w * EPW + q) * 32 + lane]);
+      unsigned nf = (flags[j] & PD_NO_FAIL) ? all : fi;
+      word |= nf << (q * R);
     }
-    nofail[moff + (int64_t)w * 32] = word;
+    int64_t wi = (off / EPW + w) * 32 + lane;
+    nofail[wi] = word & member[wi];
   }
 }
 
-__global__ void k_any_empty_row(int64_t n, const int32_t *__restrict__ rowlen, unsigned long long *out) {
+__global__ void k_checks(int64_t npad, const int32_t *__restrict__ perm, const int32_t *__restrict__ rowlen,
+                         const uint8_t *__restrict__ flags, unsigned long long *out) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  if (rowlen[i] == 0) atomicExch(&out[0], 1ull);  // some node has an empty family
-}
-
-__global__ void k_any_flag(int64_t n, const uint8_t *__restrict__ flags, unsigned long long *out) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
+  if (i >= npad || perm[i] < 0) return;
+  if (rowlen[i] == 0) atomicOr(&out[0], 1ull);  // some node has an empty family
   unsigned f = flags[i];
-  if (f & PD_NO_FAIL) atomicOr(&out[0], 1ull);
-  if (f) atomicOr(&out[0], 2ull);
-}
-
-__global__ void k_node_consts(int64_t npad, int64_t n, double G, const double *__restrict__ m, double *minv,
-                              double *gmu) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= npad) return;
-  double mi = i < n ? m[i] : 1.0;
-  minv[i] = i < n ? 1.0 / mi : 0.0;
-  gmu[i] = i < n ? G / mi : 0.0;
+  if (f & PD_NO_FAIL) atomicOr(&out[1], 1ull);
+  if (f) atomicOr(&out[1], 2ull);
 }
 
 __global__ void k_rowlen_user(int64_t n, const int32_t *__restrict__ iperm, const int32_t *__restrict__ rowlen,
@@ -305,24 +470,45 @@ __global__ void k_rowlen_user(int64_t n, const int32_t *__restrict__ iperm, cons
   out[uidx] = rowlen[iperm[uidx]];
 }
 
-__global__ void k_export_rows(int64_t n, const int32_t *__restrict__ perm, const long long *__restrict__ rowptr,
-                              const int32_t *__restrict__ rowlen, const uint32_t *__restrict__ slice_off,
-                              const uint32_t *__restrict__ mask_off, const int32_t *__restrict__ col,
-                              const uint32_t *__restrict__ mask, int32_t *col_out, uint8_t *intact_out) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  int lane = (int)(i & 31);
-  int64_t s = i >> 5;
-  int64_t off = (int64_t)slice_off[s] * 32 + lane, moff = (int64_t)mask_off[s] * 32 + lane;
-  long long base = rowptr[perm[i]];
-  int len = rowlen[i];
-  for (int k = 0; k < len; ++k) {
-    col_out[base + k] = perm[col[off + (int64_t)k * 32]];
-    intact_out[base + k] = (uint8_t)((mask[moff + (int64_t)(k >> 5) * 32] >> (k & 31)) & 1u);
+__global__ void k_export_rows(int64_t ngroups, int R, const int32_t *__restrict__ perm,
+                              const long long *__restrict__ rowptr, const uint32_t *__restrict__ goff,
+                              const uint32_t *__restrict__ col, const uint32_t *__restrict__ member,
+                              const uint32_t *__restrict__ intact, int32_t *col_out, uint8_t *intact_out) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int64_t grp = t >> 5;
+  if (grp >= ngroups) return;
+  int lane = threadIdx.x & 31;
+  const int EPW = 32 / R;
+  int64_t off = goff[grp];
+  int len = (int)(goff[grp + 1] - goff[grp]);
+  for (int r = 0; r < R; ++r) {
+    int32_t uidx = perm[(grp * R + r) * 32 + lane];
+    if (uidx < 0) continue;
+    long long base = rowptr[uidx];
+    for (int k = 0; k < len; ++k) {
+      int64_t w = (off + k) / EPW * 32 + lane;
+      uint32_t bit = 1u << ((k % EPW) * R + r);
+      if (member[w] & bit) {
+        col_out[base] = perm[pd_elem_inv(col[(off + k) * 32 + lane])];
+        intact_out[base] = (intact[w] & bit) ? 1 : 0;
+        ++base;
+      }
+    }
   }
 }
 
 inline unsigned nblk(int64_t n) { return (unsigned)((n + TPB - 1) / TPB); }
+
+template <typename T>
+int scan_exclusive(pd_sim *s, std::vector<void *> &scratch, const T *in, T *out, int64_t cnt) {
+  size_t tb = 0;
+  PD_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, tb, in, out, (int)cnt, s->stream));
+  void *tmp = pdi::dev_alloc(s, tb ? tb : 1);
+  if (!tmp) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
+  scratch.push_back(tmp);
+  PD_CUDA(cub::DeviceScan::ExclusiveSum(tmp, tb, in, out, (int)cnt, s->stream));
+  return PD_OK;
+}
 
 }  // namespace
 
@@ -339,13 +525,13 @@ int build_family(pd_sim *s, const double *coords, const double *vol, const uint8
   cudaStream_t st = s->stream;
   const int64_t n = s->n;
   const int dim = s->dim;
-  s->npad = (n + 31) / 32 * 32;
-  s->nslices = s->npad / 32;
+  const int R = s->R;
+  const int EPW = 32 / R;
 
   // ---- scratch (freed at the end through the same allocator) ----
   std::vector<void *> scratch;
   auto salloc = [&](size_t bytes) -> void * {
-    void *p = dev_alloc(s, bytes);
+    void *p = dev_alloc(s, bytes ? bytes : 1);
     if (p) scratch.push_back(p);
     return p;
   };
@@ -355,15 +541,17 @@ int build_family(pd_sim *s, const double *coords, const double *vol, const uint8
     scratch.clear();
   };
   struct Guard { decltype(sfree_all) &f; ~Guard() { f(); } } guard{sfree_all};
+#define SCRATCH(ptr, type, count)                                            \
+  type *ptr = (type *)salloc(sizeof(type) * (size_t)(count));                \
+  if (!ptr) { set_error("device allocation failed in pd_create"); return PD_ERR_ALLOC; }
 
   // ---- 1. bbox + volume range ----
-  unsigned long long *red = (unsigned long long *)salloc(8 * sizeof(unsigned long long));
-  if (!red) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
+  SCRATCH(red, unsigned long long, 8);
   unsigned long long init[8];
   for (int k = 0; k < 3; ++k) { init[k] = ~0ull; init[3 + k] = 0ull; }
   init[6] = ~0ull; init[7] = 0ull;
   PD_CUDA(cudaMemcpyAsync(red, init, sizeof(init), cudaMemcpyHostToDevice, st));
-  k_bbox<<<nblk(n), TPB, 0, st>>>(n, dim, coords, vol, red);
+  k_bbox<<<std::min<unsigned>(nblk(n), 1184u), TPB, 0, st>>>(n, dim, coords, vol, red);
   unsigned long long hred[8];
   PD_CUDA(cudaMemcpyAsync(hred, red, sizeof(hred), cudaMemcpyDeviceToHost, st));
   PD_CUDA(cudaStreamSynchronize(st));
@@ -376,129 +564,169 @@ int build_family(pd_sim *s, const double *coords, const double *vol, const uint8
   s->uniform_v = (vmin == vmax);
   s->vol_uniform = vmin;
 
-  // ---- fine cell grid: edge = horizon/kdiv (slightly enlarged so that a neighbour is never more
-  //      than kdiv cells away in spite of rounding in the cell computation) ----
-  double meas = 1.0;
-  int nd = 0;
-  for (int k = 0; k < dim; ++k)
-    if (hi[k] > lo[k]) { meas *= (hi[k] - lo[k]); ++nd; }
-  int kdiv = 1;
-  if (nd > 0) {
-    double spacing = std::pow(meas / (double)n, 1.0 / nd);
-    if (spacing > 0) kdiv = (int)std::lround(s->horizon / spacing);
+  // ---- node spacing: median nearest-neighbour distance of up to 1024 sample nodes ----
+  double spacing = s->horizon;
+  {
+    const int nsamp = (int)std::min<int64_t>(n, 1024);
+    SCRATCH(nn_d, double, nsamp);
+    k_nn_sample<<<nsamp, TPB, 0, st>>>(n, dim, coords, n / nsamp, nn_d);
+    std::vector<double> nn(nsamp);
+    PD_CUDA(cudaMemcpyAsync(nn.data(), nn_d, sizeof(double) * nsamp, cudaMemcpyDeviceToHost, st));
+    PD_CUDA(cudaStreamSynchronize(st));
+    std::vector<double> ok;
+    for (double v : nn) if (v > 0.0 && v < 1.0e299 && std::isfinite(v)) ok.push_back(std::sqrt(v));
+    if (!ok.empty()) {
+      std::nth_element(ok.begin(), ok.begin() + ok.size() / 2, ok.end());
+      spacing = ok[ok.size() / 2];
+    }
   }
-  kdiv = std::min(std::max(kdiv, 1), 4);
+  // ---- cell grid: edge_k = extent_k / round(extent_k / spacing), kept inside [horizon/8, horizon];
+  //      cell index = round((x - lo)/edge): a lattice node sits in the middle of its own cell ----
+  spacing = std::min(std::max(spacing, s->horizon / 8.0), s->horizon);
   Grid g{};
   g.dim = dim;
   for (;;) {
-    double c = (s->horizon / kdiv) * (1.0 + 1e-9);
-    g.inv_c = 1.0 / c;
     double ncell = 1.0;
     for (int k = 0; k < 3; ++k) {
       g.lo[k] = lo[k];
-      double cnt = k < dim ? std::floor((hi[k] - lo[k]) * g.inv_c) + 1.0 : 1.0;
-      ncell *= cnt;
-      g.nc[k] = cnt < 2.0e9 ? (int)cnt : 2000000000;
+      double ext = k < dim ? hi[k] - lo[k] : 0.0;
+      double cnt = std::floor(ext / spacing + 0.5);
+      double c = cnt >= 1.0 ? ext / cnt : spacing;
+      g.inv_c[k] = 1.0 / c;
+      ncell *= cnt + 1.0;
+      g.nc[k] = cnt + 1.0 < 2.0e9 ? (int)cnt + 1 : 2000000000;
+      // |round(a) - round(b)| <= floor(|a - b|) + 1
+      g.S[k] = k < dim ? (int)std::floor(s->horizon / c) + 1 : 0;
     }
     if (ncell <= (double)(1ll << 28)) break;
-    if (kdiv == 1) { set_error("cell table too large: domain extent / horizon exceeds 2^28 cells"); return PD_ERR_LIMIT; }
-    --kdiv;
+    if (spacing >= s->horizon) { set_error("cell table too large: domain extent / horizon exceeds 2^28 cells"); return PD_ERR_LIMIT; }
+    spacing = std::min(spacing * 2.0, s->horizon);
   }
-  g.R = kdiv;
-  s->kdiv = kdiv;
-  // brick = one CTA's spatial tile: 32 cells along x (one warp per row), 8 rows
-  g.B[0] = 32;
-  g.B[1] = dim == 2 ? 8 : 4;
-  g.B[2] = dim == 2 ? 1 : 2;
-  for (int k = 0; k < 3; ++k) g.nb[k] = (g.nc[k] + g.B[k] - 1) / g.B[k];
+  s->kdiv = g.S[0];
+  g.R = R;
+  g.BZ = dim == 3 ? PD_GROUPS_PER_CTA : 1;
+  g.ncyg = (g.nc[1] + R - 1) / R;
+  g.nczt = (g.nc[2] + g.BZ - 1) / g.BZ;
   const int64_t ncell = (int64_t)g.nc[0] * g.nc[1] * g.nc[2];
+  const int64_t nrow = (int64_t)g.nc[1] * g.nc[2];
+  const int64_t ntr = (int64_t)g.nczt * g.ncyg;
 
-  // ---- 2. sort by brick-raster key ----
-  unsigned long long *keys = (unsigned long long *)salloc(sizeof(unsigned long long) * n);
-  unsigned long long *keys2 = (unsigned long long *)salloc(sizeof(unsigned long long) * n);
-  int32_t *ids = (int32_t *)salloc(sizeof(int32_t) * n);
-  if (!keys || !keys2 || !ids) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
-  BUILD_ALLOC(s->perm, int32_t, n);
-  BUILD_ALLOC(s->iperm, int32_t, n);
+  // ---- 2. sort by cell id ----
+  SCRATCH(keys, uint32_t, n);
+  SCRATCH(keys2, uint32_t, n);
+  SCRATCH(ids, int32_t, n);
+  SCRATCH(ord1, int32_t, n);
   k_keys<<<nblk(n), TPB, 0, st>>>(n, g, coords, keys, ids);
   {
-    double maxkey = (double)g.nb[0] * g.nb[1] * g.nb[2] * (g.B[0] * g.B[1] * g.B[2]);
-    int bits = std::min(64, (int)std::ceil(std::log2(maxkey + 1.0)) + 1);
+    int bits = 1;
+    while (bits < 32 && (1ll << bits) < ncell) ++bits;
     size_t tb = 0;
-    PD_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, tb, keys, keys2, ids, s->perm, (int)n, 0, bits, st));
-    void *tmp = salloc(tb ? tb : 1);
+    PD_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, tb, keys, keys2, ids, ord1, (int)n, 0, bits, st));
+    void *tmp = salloc(tb);
     if (!tmp) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
-    PD_CUDA(cub::DeviceRadixSort::SortPairs(tmp, tb, keys, keys2, ids, s->perm, (int)n, 0, bits, st));
+    PD_CUDA(cub::DeviceRadixSort::SortPairs(tmp, tb, keys, keys2, ids, ord1, (int)n, 0, bits, st));
   }
-
-  // ---- node arrays in sorted order ----
-  for (int k = 0; k < 3; ++k) {
-    if (k < dim) BUILD_ALLOC(s->x[k], double, s->npad); else s->x[k] = nullptr;
-  }
-  BUILD_ALLOC(s->vol, double, s->npad);
-  BUILD_ALLOC(s->flags, uint8_t, s->npad);
-  k_gather_nodes<<<nblk(s->npad), TPB, 0, st>>>(n, s->npad, dim, s->perm, coords, vol, flags, s->x[0], s->x[1],
-                                                 s->x[2], s->vol, s->flags, s->iperm);
-
-  // ---- 3. cell table ----
-  int32_t *cell_start = (int32_t *)salloc(sizeof(int32_t) * ncell);
-  int32_t *cell_end = (int32_t *)salloc(sizeof(int32_t) * ncell);
-  if (!cell_start || !cell_end) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
+  SCRATCH(cell_start, int32_t, ncell);
+  SCRATCH(cell_end, int32_t, ncell);
+  SCRATCH(row_start, int32_t, nrow);
+  SCRATCH(row_end, int32_t, nrow);
   PD_CUDA(cudaMemsetAsync(cell_start, 0, sizeof(int32_t) * ncell, st));
   PD_CUDA(cudaMemsetAsync(cell_end, 0, sizeof(int32_t) * ncell, st));
-  k_cell_table<<<nblk(n), TPB, 0, st>>>(n, g, s->x[0], s->x[1], s->x[2], cell_start, cell_end);
+  PD_CUDA(cudaMemsetAsync(row_start, 0, sizeof(int32_t) * nrow, st));
+  PD_CUDA(cudaMemsetAsync(row_end, 0, sizeof(int32_t) * nrow, st));
+  k_tables<<<nblk(n), TPB, 0, st>>>(n, g.nc[0], keys2, cell_start, cell_end, row_start, row_end);
 
-  // ---- 4. count -> slice lengths -> offsets ----
+  // ---- 3. lanes, tiles, final order ----
+  SCRATCH(rowid, int32_t, n);
+  SCRATCH(tval, int32_t, n);
+  SCRATCH(tmax, int32_t, n);
+  SCRATCH(vx, int32_t, n);
+  SCRATCH(tile_x0, int32_t, ntr);
+  k_row_t<<<nblk(n), TPB, 0, st>>>(n, g.nc[0], keys2, row_start, rowid, tval);
+  {
+    size_t tb = 0;
+    PD_CUDA(cub::DeviceScan::InclusiveScanByKey(nullptr, tb, rowid, tval, tmax, cub::Max(), (int)n, cub::Equality(), st));
+    void *tmp = salloc(tb);
+    if (!tmp) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
+    PD_CUDA(cub::DeviceScan::InclusiveScanByKey(tmp, tb, rowid, tval, tmax, cub::Max(), (int)n, cub::Equality(), st));
+  }
+  k_tilerow_x0<<<nblk(ntr), TPB, 0, st>>>(ntr, g, keys2, row_start, row_end, tile_x0);
+  int *maxvx_d = (int *)(red + 2);
+  PD_CUDA(cudaMemsetAsync(red, 0, 8 * sizeof(unsigned long long), st));
+  k_vx<<<nblk(n), TPB, 0, st>>>(n, g, rowid, row_start, tmax, tile_x0, vx, maxvx_d);
+  int maxvx = 0;
+  PD_CUDA(cudaMemcpyAsync(&maxvx, maxvx_d, sizeof(int), cudaMemcpyDeviceToHost, st));
+  PD_CUDA(cudaStreamSynchronize(st));
+  g.maxchunk = maxvx / 32 + 1;
+
+  const int64_t ntile_dense = ntr * g.maxchunk;
+  if (ntile_dense >= (1ll << 31) - 1) { set_error("tile table too large"); return PD_ERR_LIMIT; }
+  SCRATCH(tile_flag, int32_t, ntile_dense + 1);
+  SCRATCH(tile_ord, int32_t, ntile_dense + 1);
+  PD_CUDA(cudaMemsetAsync(tile_flag, 0, sizeof(int32_t) * (ntile_dense + 1), st));
+  k_tile_mark<<<nblk(n), TPB, 0, st>>>(n, g, rowid, vx, tile_flag);
+  {
+    int rc = scan_exclusive<int32_t>(s, scratch, tile_flag, tile_ord, ntile_dense + 1);
+    if (rc) return rc;
+  }
+  int32_t ntile = 0;
+  PD_CUDA(cudaMemcpyAsync(&ntile, tile_ord + ntile_dense, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  PD_CUDA(cudaStreamSynchronize(st));
+  s->ngroups = (int64_t)ntile * g.BZ;
+  s->nslices = s->ngroups * R;
+  s->npad = s->nslices * 32;
+  if (s->npad >= (1ll << 31) - 64 || s->npad * PD_NF >= (1ll << 32)) { set_error("too many nodes after padding"); return PD_ERR_LIMIT; }
+
+  SCRATCH(fin1, int32_t, n);
+  SCRATCH(tile_inv, int32_t, ntile);
+  BUILD_ALLOC(s->perm, int32_t, s->npad);
+  BUILD_ALLOC(s->iperm, int32_t, n);
+  PD_CUDA(cudaMemsetAsync(s->perm, 0xff, sizeof(int32_t) * s->npad, st));
+  k_final_index<<<nblk(n), TPB, 0, st>>>(n, g, rowid, vx, ord1, tile_ord, tile_inv, fin1, s->perm, s->iperm);
+
+  BUILD_ALLOC(s->rec, double, s->npad * PD_NF);
+  BUILD_ALLOC(s->flags, uint8_t, s->npad);
+  PD_CUDA(cudaMemsetAsync(s->rec, 0, sizeof(double) * s->npad * PD_NF, st));
+  PD_CUDA(cudaMemsetAsync(s->flags, 0, s->npad, st));
+  k_records<<<nblk(s->npad), TPB, 0, st>>>(s->npad, dim, s->perm, coords, vol, flags, s->rec, s->flags);
+
+  // ---- 4. count -> group lengths -> offsets ----
   const double h2 = s->horizon * s->horizon;
   BUILD_ALLOC(s->rowlen, int32_t, s->npad);
-  BUILD_ALLOC(s->slice_len, int32_t, s->nslices);
-  BUILD_ALLOC(s->slice_off, uint32_t, s->nslices + 1);
-  BUILD_ALLOC(s->mask_off, uint32_t, s->nslices + 1);
-  int32_t *slice_words = (int32_t *)salloc(sizeof(int32_t) * s->nslices);
-  if (!slice_words) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
-  k_count<<<nblk(s->npad), TPB, 0, st>>>(n, s->npad, g, h2, s->x[0], s->x[1], s->x[2], cell_start, cell_end,
-                                          s->rowlen, s->slice_len, slice_words);
-  {
-    size_t tb1 = 0, tb2 = 0;
-    PD_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, tb1, s->slice_len, s->slice_off, (int)s->nslices, st));
-    PD_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, tb2, slice_words, s->mask_off, (int)s->nslices, st));
-    size_t tb = std::max(tb1, tb2);
-    void *tmp = salloc(tb ? tb : 1);
-    if (!tmp) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
-    // widen on the fly: inputs are int32 lengths, outputs uint32 offsets (in slots)
-    PD_CUDA(cub::DeviceScan::ExclusiveSum(tmp, tb, s->slice_len, s->slice_off, (int)s->nslices, st));
-    PD_CUDA(cub::DeviceScan::ExclusiveSum(tmp, tb, slice_words, s->mask_off, (int)s->nslices, st));
+  BUILD_ALLOC(s->goff, uint32_t, s->ngroups + 1);
+  SCRATCH(glen, uint32_t, s->ngroups + 1);
+  PD_CUDA(cudaMemsetAsync(glen + s->ngroups, 0, sizeof(uint32_t), st));
+  const unsigned gblk = nblk(s->ngroups * 32);
+  switch (R) {
+    case 1: k_count<1><<<gblk, TPB, 0, st>>>(s->ngroups, g, h2, s->rec, s->perm, cell_start, cell_end, fin1, tile_inv, tile_x0, s->rowlen, glen); break;
+    case 2: k_count<2><<<gblk, TPB, 0, st>>>(s->ngroups, g, h2, s->rec, s->perm, cell_start, cell_end, fin1, tile_inv, tile_x0, s->rowlen, glen); break;
+    default: k_count<4><<<gblk, TPB, 0, st>>>(s->ngroups, g, h2, s->rec, s->perm, cell_start, cell_end, fin1, tile_inv, tile_x0, s->rowlen, glen); break;
   }
-  // totals (last offset + last length) and the sum of row lengths
-  uint32_t last_off[2];
-  int32_t last_len[2];
-  PD_CUDA(cudaMemcpyAsync(&last_off[0], s->slice_off + (s->nslices - 1), 4, cudaMemcpyDeviceToHost, st));
-  PD_CUDA(cudaMemcpyAsync(&last_off[1], s->mask_off + (s->nslices - 1), 4, cudaMemcpyDeviceToHost, st));
-  PD_CUDA(cudaMemcpyAsync(&last_len[0], s->slice_len + (s->nslices - 1), 4, cudaMemcpyDeviceToHost, st));
-  PD_CUDA(cudaMemcpyAsync(&last_len[1], slice_words + (s->nslices - 1), 4, cudaMemcpyDeviceToHost, st));
-  long long *zsum = (long long *)salloc(sizeof(long long));
-  if (!zsum) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
   {
-    // int32 row lengths summed into a 64-bit accumulator
+    int rc = scan_exclusive<uint32_t>(s, scratch, glen, s->goff, s->ngroups + 1);
+    if (rc) return rc;
+  }
+  uint32_t total_entries = 0;
+  PD_CUDA(cudaMemcpyAsync(&total_entries, s->goff + s->ngroups, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+  SCRATCH(zsum, long long, 1);
+  {
     cub::TransformInputIterator<long long, cub::CastOp<long long>, const int32_t *> it(s->rowlen, cub::CastOp<long long>());
     size_t tb = 0;
     PD_CUDA(cub::DeviceReduce::Sum(nullptr, tb, it, zsum, (int)s->npad, st));
-    void *tmp = salloc(tb ? tb : 1);
+    void *tmp = salloc(tb);
     if (!tmp) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
     PD_CUDA(cub::DeviceReduce::Sum(tmp, tb, it, zsum, (int)s->npad, st));
   }
   long long hz = 0;
   PD_CUDA(cudaMemcpyAsync(&hz, zsum, sizeof(long long), cudaMemcpyDeviceToHost, st));
   PD_CUDA(cudaMemsetAsync(red, 0, 8 * sizeof(unsigned long long), st));
-  k_any_empty_row<<<nblk(n), TPB, 0, st>>>(n, s->rowlen, red);
-  if (flags) k_any_flag<<<nblk(n), TPB, 0, st>>>(n, flags, red + 1);
+  k_checks<<<nblk(s->npad), TPB, 0, st>>>(s->npad, s->perm, s->rowlen, s->flags, red);
   PD_CUDA(cudaMemcpyAsync(hred, red, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
   PD_CUDA(cudaStreamSynchronize(st));
   s->Z = hz;
-  s->nslots = (int64_t)last_off[0] + last_len[0];
-  s->nmaskwords = (int64_t)last_off[1] + last_len[1];
+  s->nentries = total_entries;
   if (hred[0]) { set_error("a node has an empty family (m_i = 0); enlarge the horizon"); return PD_ERR_ISOLATED; }
-  if (s->nslots >= (1ll << 32) - 4096 || s->Z >= (1ll << 31)) {
+  if (s->Z >= (1ll << 31)) {
     set_error("more than 2^31 directed bonds");
     return PD_ERR_LIMIT;
   }
@@ -506,30 +734,28 @@ int build_family(pd_sim *s, const double *coords, const double *vol, const uint8
   s->has_bc = (hred[1] & 2ull) != 0;
 
   // ---- 5. fill ----
-  BUILD_ALLOC(s->col, int32_t, s->nslots * 32);
-  BUILD_ALLOC(s->mask, uint32_t, s->nmaskwords * 32);
-  BUILD_ALLOC(s->fvol, double, s->npad);
-  BUILD_ALLOC(s->minv, double, s->npad);
-  BUILD_ALLOC(s->gmu, double, s->npad);
-  BUILD_ALLOC(s->m, double, s->npad);
-  double *mtmp = s->m;
-  k_fill<<<nblk(s->npad), TPB, 0, st>>>(n, s->npad, g, h2, s->x[0], s->x[1], s->x[2], s->vol, cell_start, cell_end,
-                                         s->slice_len, s->slice_off, s->mask_off, s->col, s->mask, mtmp, s->fvol);
-  k_node_consts<<<nblk(s->npad), TPB, 0, st>>>(s->npad, n, s->G, mtmp, s->minv, s->gmu);
+  const size_t nwords = (size_t)(total_entries / EPW) * 32;
+  BUILD_ALLOC(s->col, uint32_t, (size_t)total_entries * 32 + 32);
+  BUILD_ALLOC(s->member, uint32_t, nwords + 32);
+  BUILD_ALLOC(s->intact, uint32_t, nwords + 32);
+  switch (R) {
+    case 1: k_fill<1><<<gblk, TPB, 0, st>>>(s->ngroups, g, h2, s->G, s->rec, s->perm, cell_start, cell_end, fin1, tile_inv, tile_x0, s->goff, s->col, s->member); break;
+    case 2: k_fill<2><<<gblk, TPB, 0, st>>>(s->ngroups, g, h2, s->G, s->rec, s->perm, cell_start, cell_end, fin1, tile_inv, tile_x0, s->goff, s->col, s->member); break;
+    default: k_fill<4><<<gblk, TPB, 0, st>>>(s->ngroups, g, h2, s->G, s->rec, s->perm, cell_start, cell_end, fin1, tile_inv, tile_x0, s->goff, s->col, s->member); break;
+  }
+  PD_CUDA(cudaMemcpyAsync(s->intact, s->member, sizeof(uint32_t) * nwords, cudaMemcpyDeviceToDevice, st));
 
   // ---- 6. pre-cuts, no-fail ----
   if (n_precut > 0) {
     PD_CUDA(cudaMemsetAsync(red, 0, sizeof(unsigned long long), st));
-    k_precut<<<nblk(2 * n_precut), TPB, 0, st>>>(n_precut, n, precut, s->iperm, s->rowlen, s->slice_off, s->mask_off,
-                                                  s->col, s->mask, red);
+    k_precut<<<nblk(2 * n_precut), TPB, 0, st>>>(n_precut, n, R, precut, s->iperm, s->goff, s->col, s->member, s->intact, red);
     PD_CUDA(cudaMemcpyAsync(hred, red, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     PD_CUDA(cudaStreamSynchronize(st));
     if (hred[0]) { set_error("a pre-cut pair is out of range or not a bond"); return PD_ERR_ARG; }
   }
   if (s->has_nofail && s->fracture) {
-    BUILD_ALLOC(s->nofail, uint32_t, s->nmaskwords * 32);
-    k_nofail<<<nblk(s->npad), TPB, 0, st>>>(s->npad, s->flags, s->rowlen, s->slice_len, s->slice_off, s->mask_off,
-                                             s->col, s->nofail);
+    BUILD_ALLOC(s->nofail, uint32_t, nwords + 32);
+    k_nofail<<<gblk, TPB, 0, st>>>(s->ngroups, R, s->flags, s->goff, s->col, s->member, s->nofail);
   }
   PD_CUDA(cudaGetLastError());
   PD_CUDA(cudaStreamSynchronize(st));
@@ -553,8 +779,8 @@ int export_bond_mask(pd_sim *s, long long *rowptr_dev, int32_t *col_dev, uint8_t
     if (!tmp) { set_error("device allocation failed"); rc = PD_ERR_ALLOC; break; }
     if (cub::DeviceScan::ExclusiveSum(tmp, tb, cnt, rowptr_dev, (int)(n + 1), st) != cudaSuccess) { rc = PD_ERR_CUDA; break; }
     if (col_dev && intact_dev)
-      k_export_rows<<<nblk(n), TPB, 0, st>>>(n, s->perm, rowptr_dev, s->rowlen, s->slice_off, s->mask_off, s->col,
-                                              s->mask, col_dev, intact_dev);
+      k_export_rows<<<nblk(s->ngroups * 32), TPB, 0, st>>>(s->ngroups, s->R, s->perm, rowptr_dev, s->goff, s->col,
+                                                            s->member, s->intact, col_dev, intact_dev);
     if (cudaGetLastError() != cudaSuccess) rc = PD_ERR_CUDA;
   } while (0);
   cudaStreamSynchronize(st);

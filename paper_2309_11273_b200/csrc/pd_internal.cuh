@@ -1,13 +1,27 @@
 // pd_internal.cuh -- private state of libpd.so (not part of the boundary; see include/pd.h).
 //
-// Data layout in HBM (all node arrays in the library's SORTED node order, padded to a
-// multiple of 32 nodes):
-//   x[k], u[b][k], v[k], bval[k] : SoA FP64, one array per component k (u double-buffered, b = 0/1)
-//   vol, minv (=1/m_i), gmu (=G/m_i), cth (=(K-G/3) theta_i/m_i, rewritten every step), fvol
-//   sliced ELL ("SELL-32"): slice s = sorted nodes 32s .. 32s+31 (one warp, one lane per node);
-//     col [(slice_off[s] + k)*32 + lane]  : neighbour (sorted index) in slot k of that lane's row
-//     mask[(mask_off[s]  + w)*32 + lane]  : bit b of word w = bond in slot 32w+b intact (Eq. 1.30)
-//   slots past a row's length point at the node itself and have mask bit 0.
+// Data layout in HBM.  Nodes are renumbered by the builder into a
+// FINAL order made of 32-node SLICES (one warp lane per node); R consecutive slices form a
+// GROUP (one warp): lane l of group g owns the R nodes (g*R + r)*32 + l, r = 0..R-1, which the
+// builder chooses to be the l-th nodes of R adjacent lattice rows.  Missing nodes are PHANTOMS
+// (perm = -1, zero record, no bonds).
+//
+//   rec : node records, AoSoA-32 with PD_NF = 16 FP64 fields per node:
+//         element index elem(i) = (i >> 5) * (32*PD_NF) + (i & 31); field f lives at elem + 32 f
+//         (so a warp reads 256 contiguous bytes per field and one address serves all fields).
+//         fields: 0-2 x (reference position)   3 gmu = G/m_i      4 vol = V_i     5 minv = 1/m_i
+//                 6 m_i                        7 fvol = sum_j V_j
+//                 8-10 u (buffer 0)  11 cth (buffer 0)   12-14 u (buffer 1)  15 cth (buffer 1)
+//         cth_i = (K - G/3) theta_i / m_i belongs to the u buffer it was computed from.
+//   blocked sliced ELL ("SELL-32xR"): group g has glen[g] ENTRIES starting at goff[g]; entry k of
+//         lane l is ONE neighbour shared by the lane's R nodes:
+//           col   [(goff[g] + k)*32 + l]            elem() of the neighbour
+//           intact[(goff[g] + k)/EPW*32 + l]        bit ((k % EPW)*R + r): bond (node r, neighbour)
+//                                                   exists and is unbroken (Eq. 1.30); EPW = 32/R
+//           member[...]  same shape, static: the bond exists (family membership)
+//           nofail[...]  same shape, static, only if some node is no-fail
+//         padding entries point at the lane's own node 0 and have all bits 0.
+//   v, bval : SoA [dim][npad];  flags, rowlen, phi : [npad]
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -18,13 +32,30 @@
 #include "../../include/pd.h"
 
 #define PD_MAX_DIM 3
-#define PD_SLOT_ALIGN 4  // slice lengths are rounded up to a multiple of this (inner unroll)
+#define PD_NF 16          // FP64 fields per node record
+#define PD_F_X 0
+#define PD_F_GMU 3
+#define PD_F_VOL 4
+#define PD_F_MINV 5
+#define PD_F_M 6
+#define PD_F_FVOL 7
+#define PD_F_U(buf) (8 + 4 * (buf))
+#define PD_F_CTH(buf) (11 + 4 * (buf))
+#define PD_GROUPS_PER_CTA 4   // 128 threads; in 3D the 4 groups of a CTA are 4 z-levels of one tile
+
+__host__ __device__ __forceinline__ uint32_t pd_elem(int64_t i) {
+  return (uint32_t)((i >> 5) * (32 * PD_NF) + (i & 31));
+}
+__host__ __device__ __forceinline__ int64_t pd_elem_inv(uint32_t e) {
+  return ((int64_t)(e / (32 * PD_NF)) << 5) | (e & 31);
+}
 
 struct pd_sim {
   // scalars
   int dim = 0, mode = 0;
-  int64_t n = 0, npad = 0, nslices = 0;
-  int64_t Z = 0, nslots = 0, nmaskwords = 0;  // directed bonds, stored slots (per lane), mask words (per lane)
+  int R = 4;                    // rows (nodes) per thread
+  int64_t n = 0, npad = 0, nslices = 0, ngroups = 0;
+  int64_t Z = 0, nentries = 0;  // directed bonds; stored entries per lane (sum of glen)
   double horizon = 0, A = 0, K = 0, G = 0, c1 = 0;  // c1 = K - G/3
   double rho = 0, dt = 0, s_c = 0, ramp_time = 0, vol_uniform = 0;
   bool fracture = false, uniform_v = false, has_nofail = false, has_bc = false;
@@ -35,23 +66,23 @@ struct pd_sim {
   cudaStream_t stream = 0;
   std::vector<std::pair<void *, size_t>> allocs;
   size_t bytes_held = 0;
-  // node arrays (sorted order)
-  int32_t *perm = nullptr, *iperm = nullptr;  // perm[sorted] = user, iperm[user] = sorted
-  double *x[PD_MAX_DIM] = {}, *u[2][PD_MAX_DIM] = {}, *v[PD_MAX_DIM] = {}, *bval[PD_MAX_DIM] = {};
-  double *vol = nullptr, *m = nullptr, *minv = nullptr, *gmu = nullptr, *cth = nullptr, *fvol = nullptr, *phi = nullptr;
+  // node arrays (final order)
+  int32_t *perm = nullptr, *iperm = nullptr;  // perm[final] = user or -1, iperm[user] = final
+  double *rec = nullptr;
+  double *v[PD_MAX_DIM] = {}, *bval[PD_MAX_DIM] = {};
+  double *phi = nullptr;
   uint8_t *flags = nullptr;
   int32_t *rowlen = nullptr;
-  // SELL
-  uint32_t *slice_off = nullptr, *mask_off = nullptr;
-  int32_t *slice_len = nullptr;
-  int32_t *col = nullptr;
-  uint32_t *mask = nullptr, *nofail = nullptr;
+  // blocked SELL
+  uint32_t *goff = nullptr;   // [ngroups + 1] entry offsets (multiples of EPW)
+  uint32_t *col = nullptr;
+  uint32_t *intact = nullptr, *member = nullptr, *nofail = nullptr;
   // state
   int cur = 0;            // which u buffer holds u^n
   int64_t step = 0;       // n
   int64_t launches = 0;   // kernels launched by pd_step
   bool break_pending = false;  // u^n has not been break-checked yet (deferred step 5)
-  unsigned long long *stats_dev = nullptr;  // [0]=broken directed, [1]=max phi bits, [2]=#phi>=.5, [3]=err flag
+  unsigned long long *stats_dev = nullptr;  // [0]=broken directed, [1]=max phi bits, [2]=#phi>=.5
 };
 
 namespace pdi {
@@ -65,9 +96,9 @@ int build_family(pd_sim *s, const double *coords_user_dev, const double *vol_use
                  const uint8_t *flags_user_dev, const int32_t *precut_dev, int64_t n_precut);
 int export_bond_mask(pd_sim *s, long long *rowptr_dev, int32_t *col_dev, uint8_t *intact_dev);
 // pd_step.cu
-void launch_dilatation(pd_sim *s, const double *const *ucur, double *theta_out, bool do_break);
-void launch_force_update(pd_sim *s);
-void launch_damage(pd_sim *s);
+int launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
+int launch_force_update(pd_sim *s);
+int launch_damage(pd_sim *s);
 }  // namespace pdi
 
 #define PD_CUDA(call)                                                       \
