@@ -14,7 +14,8 @@ constexpr int TPB = 256;
 inline unsigned nblk(int64_t n) { return (unsigned)((n + TPB - 1) / TPB); }
 
 // user AoS (dim*n) -> final order; dst is either a record field (stride 32, via pd_elem) or SoA arrays
-__global__ void k_scatter_field(int64_t npad, int dim, const int32_t *__restrict__ perm, const double *__restrict__ src,
+struct Ax { int a[3]; };
+__global__ void k_scatter_field(int64_t npad, int dim, Ax ax, const int32_t *__restrict__ perm, const double *__restrict__ src,
                                 const uint8_t *__restrict__ flags, bool clamp_zero, double *rec, int field, double *d0,
                                 double *d1, double *d2) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -23,14 +24,14 @@ __global__ void k_scatter_field(int64_t npad, int dim, const int32_t *__restrict
   int32_t uidx = perm[i];
   unsigned fl = flags[i];
   for (int k = 0; k < dim; ++k) {
-    double val = (src && uidx >= 0) ? src[(int64_t)dim * uidx + k] : 0.0;
+    double val = (src && uidx >= 0) ? src[(int64_t)dim * uidx + ax.a[k]] : 0.0;
     if (clamp_zero && (fl & (1u << k))) val = 0.0;
     if (rec) rec[pd_elem(i) + 32 * (field + k)] = val; else d[k][i] = val;
   }
 }
 
 // final order -> user AoS; source is a record field or SoA arrays
-__global__ void k_gather_field(int64_t npad, int dim, const int32_t *__restrict__ perm, const double *__restrict__ rec,
+__global__ void k_gather_field(int64_t npad, int dim, Ax ax, const int32_t *__restrict__ perm, const double *__restrict__ rec,
                                int field, const double *__restrict__ s0, const double *__restrict__ s1,
                                const double *__restrict__ s2, double *dst) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -38,7 +39,7 @@ __global__ void k_gather_field(int64_t npad, int dim, const int32_t *__restrict_
   const double *s[3] = {s0, s1, s2};
   int32_t uidx = perm[i];
   if (uidx < 0) return;
-  for (int k = 0; k < dim; ++k) dst[(int64_t)dim * uidx + k] = rec ? rec[pd_elem(i) + 32 * (field + k)] : s[k][i];
+  for (int k = 0; k < dim; ++k) dst[(int64_t)dim * uidx + ax.a[k]] = rec ? rec[pd_elem(i) + 32 * (field + k)] : s[k][i];
 }
 
 // scalar per node: record field (rec != NULL) or plain array
@@ -92,7 +93,7 @@ int get_field(pd_sim *s, double *dst, int field /* record field, or -1 = velocit
   if (!s || !dst) { pdi::set_error("null argument"); return PD_ERR_ARG; }
   DevTmp tmp(s, sizeof(double) * s->dim * s->n);
   if (!tmp.p) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
-  k_gather_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->dim, s->perm, field >= 0 ? s->rec : nullptr, field,
+  k_gather_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, field >= 0 ? s->rec : nullptr, field,
                                                        s->v[0], s->v[1], s->v[2], (double *)tmp.p);
   PD_CUDA(cudaGetLastError());
   return copy_out(s, dst, tmp.p, sizeof(double) * s->dim * s->n);
@@ -212,11 +213,11 @@ int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volum
     ok = s->stats_dev != nullptr;
   }
   if (!ok) { pdi::set_error("device allocation failed for the state arrays"); return fail(PD_ERR_ALLOC); }
-  k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, s->perm, (const double *)d_u0, s->flags, true,
+  k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, (const double *)d_u0, s->flags, true,
                                                          s->rec, PD_F_U(0), nullptr, nullptr, nullptr);
-  k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, s->perm, (const double *)d_v0, s->flags, true,
+  k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, (const double *)d_v0, s->flags, true,
                                                          nullptr, 0, s->v[0], s->v[1], s->v[2]);
-  k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, s->perm, (const double *)d_val, s->flags, false,
+  k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, (const double *)d_val, s->flags, false,
                                                          nullptr, 0, s->bval[0], s->bval[1], s->bval[2]);
   cudaError_t e = cudaGetLastError();
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);

@@ -31,6 +31,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 
 #include "pd_internal.cuh"
@@ -45,6 +46,7 @@ struct Grid {
   int nc[3];        // cells per dim
   int S[3];         // search radius in cells per dim
   int dim;
+  int ax[3];        // internal axis k = user axis ax[k]
   int R, BZ;        // rows per thread, z-levels per tile
   int ncyg, nczt, maxchunk;
 };
@@ -141,7 +143,7 @@ __global__ void k_keys(int64_t n, Grid g, const double *__restrict__ coords, uin
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   double p[3] = {0, 0, 0};
-  for (int k = 0; k < g.dim; ++k) p[k] = coords[g.dim * i + k];
+  for (int k = 0; k < g.dim; ++k) p[k] = coords[g.dim * i + g.ax[k]];
   int q[3];
   cell_of(g, p, q);
   keys[i] = (uint32_t)(((int64_t)q[2] * g.nc[1] + q[1]) * g.nc[0] + q[0]);
@@ -237,17 +239,23 @@ __global__ void k_final_index(int64_t n, Grid g, const int32_t *__restrict__ row
 }
 
 // node records in final order (rec, flags pre-zeroed; phantoms stay zero)
-__global__ void k_records(int64_t npad, int dim, const int32_t *__restrict__ perm, const double *__restrict__ coords,
+__global__ void k_records(int64_t npad, Grid g, const int32_t *__restrict__ perm, const double *__restrict__ coords,
                           const double *__restrict__ vol, const uint8_t *__restrict__ flags, double *rec,
                           uint8_t *flagsF) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= npad) return;
   int32_t uidx = perm[i];
   if (uidx < 0) return;
+  const int dim = g.dim;
   double *r = rec + pd_elem(i);
-  for (int k = 0; k < dim; ++k) r[32 * (PD_F_X + k)] = coords[(int64_t)dim * uidx + k];
+  for (int k = 0; k < dim; ++k) r[32 * (PD_F_X + k)] = coords[(int64_t)dim * uidx + g.ax[k]];
   r[32 * PD_F_VOL] = vol[uidx];
-  flagsF[i] = flags ? flags[uidx] : (uint8_t)0;
+  unsigned f = flags ? flags[uidx] : 0u, fi = f & 0xC0u;   // per-dof bits move with their component
+  for (int k = 0; k < dim; ++k) {
+    if (f & (1u << g.ax[k])) fi |= 1u << k;
+    if (f & (8u << g.ax[k])) fi |= 8u << k;
+  }
+  flagsF[i] = (uint8_t)fi;
 }
 
 // ---- 4./5. lockstep family traversal of one group (one warp; lane = R nodes) -----------------------
@@ -583,8 +591,27 @@ int build_family(pd_sim *s, const double *coords, const double *vol, const uint8
   // ---- cell grid: edge_k = extent_k / round(extent_k / spacing), kept inside [horizon/8, horizon];
   //      cell index = round((x - lo)/edge): a lattice node sits in the middle of its own cell ----
   spacing = std::min(std::max(spacing, s->horizon / 8.0), s->horizon);
+  // lane axis = the axis whose cell count fills whole 32-lane chunks best (ties: the longer one)
+  {
+    int best = 0;
+    double bfill = -1.0, bcnt = 0.0;
+    for (int k = 0; k < dim; ++k) {
+      double cnt = std::floor((hi[k] - lo[k]) / spacing + 0.5) + 1.0;
+      double fill = cnt / (32.0 * std::ceil(cnt / 32.0));
+      if (fill > bfill + 1e-12 || (std::fabs(fill - bfill) <= 1e-12 && cnt > bcnt)) { best = k; bfill = fill; bcnt = cnt; }
+    }
+    if (const char *env = getenv("PD_LANE_AXIS")) { int a = atoi(env); if (a >= 0 && a < dim) best = a; }
+    int q = 0;
+    s->ax[q++] = best;
+    for (int k = 0; k < dim; ++k) if (k != best) s->ax[q++] = k;
+    for (; q < 3; ++q) s->ax[q] = q;
+    double lo2[3] = {0, 0, 0}, hi2[3] = {0, 0, 0};
+    for (int k = 0; k < dim; ++k) { lo2[k] = lo[s->ax[k]]; hi2[k] = hi[s->ax[k]]; }
+    for (int k = 0; k < 3; ++k) { lo[k] = lo2[k]; hi[k] = hi2[k]; }
+  }
   Grid g{};
   g.dim = dim;
+  for (int k = 0; k < 3; ++k) g.ax[k] = s->ax[k];
   for (;;) {
     double ncell = 1.0;
     for (int k = 0; k < 3; ++k) {
@@ -688,7 +715,7 @@ int build_family(pd_sim *s, const double *coords, const double *vol, const uint8
   BUILD_ALLOC(s->flags, uint8_t, s->npad);
   PD_CUDA(cudaMemsetAsync(s->rec, 0, sizeof(double) * s->npad * PD_NF, st));
   PD_CUDA(cudaMemsetAsync(s->flags, 0, s->npad, st));
-  k_records<<<nblk(s->npad), TPB, 0, st>>>(s->npad, dim, s->perm, coords, vol, flags, s->rec, s->flags);
+  k_records<<<nblk(s->npad), TPB, 0, st>>>(s->npad, g, s->perm, coords, vol, flags, s->rec, s->flags);
 
   // ---- 4. count -> group lengths -> offsets ----
   const double h2 = s->horizon * s->horizon;

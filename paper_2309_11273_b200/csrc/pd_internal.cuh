@@ -9,6 +9,8 @@
 //   rec : node records, AoSoA-32 with PD_NF = 16 FP64 fields per node:
 //         element index elem(i) = (i >> 5) * (32*PD_NF) + (i & 31); field f lives at elem + 32 f
 //         (so a warp reads 256 contiguous bytes per field and one address serves all fields).
+//         (vector components are stored in INTERNAL order: component k = user component ax[k],
+//          internal axis 0 = the lane axis chosen by the builder)
 //         fields: 0-2 x (reference position)   3 gmu = G/m_i      4 vol = V_i     5 minv = 1/m_i
 //                 6 m_i                        7 fvol = sum_j V_j
 //                 8-10 u (buffer 0)  11 cth (buffer 0)   12-14 u (buffer 1)  15 cth (buffer 1)
@@ -54,6 +56,7 @@ struct pd_sim {
   // scalars
   int dim = 0, mode = 0;
   int R = 4;                    // rows (nodes) per thread
+  int ax[3] = {0, 1, 2};        // internal component k = user component ax[k]; internal 0 is the lane axis
   int64_t n = 0, npad = 0, nslices = 0, ngroups = 0;
   int64_t Z = 0, nentries = 0;  // directed bonds; stored entries per lane (sum of glen)
   double horizon = 0, A = 0, K = 0, G = 0, c1 = 0;  // c1 = K - G/3

@@ -154,16 +154,17 @@ __global__ void __launch_bounds__(TPB) k_dilatation(StepArgs a) {
             eta[k] = uj[k] - ui_[r][k];
           }
           const double dot = dot_xi_eta<DIM>(xi, eta);
-          bool b = (mw & bit) != 0;
+          const bool in = (mw & bit) != 0;
+          bool brk = false;
           if (FRAC) {
-            const double r2 = dot_xi_eta<DIM>(xi, xi);
-            if (b && dot >= a.s_c * r2 && !(nf & bit)) {  // s >= s_c breaks (Eq. 1.30)
-              mw &= ~bit;
-              b = false;
-            }
+            // s >= s_c breaks (Eq. 1.30): xi.eta - s_c ||xi||^2 >= 0, one rounding, sign read off the high word
+            const double t = fma(-a.s_c, dot_xi_eta<DIM>(xi, xi), dot);
+            brk = in && __double2hiint(t) >= 0 && !(nf & bit);
+            if (brk) mw ^= bit;
           }
-          if (UNIV) acc[r] = b ? acc[r] + dot : acc[r];
-          else acc[r] = b ? fma(vj, dot, acc[r]) : acc[r];
+          if (in && !brk) {
+            if (UNIV) acc[r] += dot; else acc[r] = fma(vj, dot, acc[r]);
+          }
         }
       }
     }
