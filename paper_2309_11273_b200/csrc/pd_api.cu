@@ -13,10 +13,11 @@ thread_local std::string g_err;
 constexpr int TPB = 256;
 inline unsigned nblk(int64_t n) { return (unsigned)((n + TPB - 1) / TPB); }
 
-// user AoS (dim*n) -> final order; dst is either a record field (stride 32, via pd_elem) or SoA arrays
+// user AoS (dim*n) -> final order; dst is either the u half of the position pairs of a neighbour-record
+// buffer (nb != NULL) or SoA arrays
 struct Ax { int a[3]; };
 __global__ void k_scatter_field(int64_t npad, int dim, Ax ax, const int32_t *__restrict__ perm, const double *__restrict__ src,
-                                const uint8_t *__restrict__ flags, bool clamp_zero, double *rec, int field, double *d0,
+                                const uint8_t *__restrict__ flags, bool clamp_zero, double2 *nb, double *d0,
                                 double *d1, double *d2) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= npad) return;
@@ -26,30 +27,29 @@ __global__ void k_scatter_field(int64_t npad, int dim, Ax ax, const int32_t *__r
   for (int k = 0; k < dim; ++k) {
     double val = (src && uidx >= 0) ? src[(int64_t)dim * uidx + ax.a[k]] : 0.0;
     if (clamp_zero && (fl & (1u << k))) val = 0.0;
-    if (rec) rec[pd_elem(i) + 32 * (field + k)] = val; else d[k][i] = val;
+    if (nb) nb[pd_elem(i) + 32 * k].y = val; else d[k][i] = val;
   }
 }
 
-// final order -> user AoS; source is a record field or SoA arrays
-__global__ void k_gather_field(int64_t npad, int dim, Ax ax, const int32_t *__restrict__ perm, const double *__restrict__ rec,
-                               int field, const double *__restrict__ s0, const double *__restrict__ s1,
+// final order -> user AoS; source is the u half of a neighbour-record buffer or SoA arrays
+__global__ void k_gather_field(int64_t npad, int dim, Ax ax, const int32_t *__restrict__ perm, const double2 *__restrict__ nb,
+                               const double *__restrict__ s0, const double *__restrict__ s1,
                                const double *__restrict__ s2, double *dst) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= npad) return;
   const double *s[3] = {s0, s1, s2};
   int32_t uidx = perm[i];
   if (uidx < 0) return;
-  for (int k = 0; k < dim; ++k) dst[(int64_t)dim * uidx + ax.a[k]] = rec ? rec[pd_elem(i) + 32 * (field + k)] : s[k][i];
+  for (int k = 0; k < dim; ++k) dst[(int64_t)dim * uidx + ax.a[k]] = nb ? nb[pd_elem(i) + 32 * k].y : s[k][i];
 }
 
-// scalar per node: record field (rec != NULL) or plain array
-__global__ void k_gather_scalar(int64_t npad, const int32_t *__restrict__ perm, const double *__restrict__ rec, int field,
-                                const double *__restrict__ src, double *dst) {
+// scalar per node
+__global__ void k_gather_scalar(int64_t npad, const int32_t *__restrict__ perm, const double *__restrict__ src, double *dst) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= npad) return;
   int32_t uidx = perm[i];
   if (uidx < 0) return;
-  dst[uidx] = rec ? rec[pd_elem(i) + 32 * field] : src[i];
+  dst[uidx] = src[i];
 }
 
 struct DevTmp {  // RAII temp allocation through the sim's allocator
@@ -89,11 +89,11 @@ int copy_out(pd_sim *s, void *dst, const void *src_dev, size_t bytes) {
   return PD_OK;
 }
 
-int get_field(pd_sim *s, double *dst, int field /* record field, or -1 = velocity arrays */) {
+int get_field(pd_sim *s, double *dst, bool velocity) {
   if (!s || !dst) { pdi::set_error("null argument"); return PD_ERR_ARG; }
   DevTmp tmp(s, sizeof(double) * s->dim * s->n);
   if (!tmp.p) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
-  k_gather_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, field >= 0 ? s->rec : nullptr, field,
+  k_gather_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, velocity ? nullptr : s->nb[s->cur],
                                                        s->v[0], s->v[1], s->v[2], (double *)tmp.p);
   PD_CUDA(cudaGetLastError());
   return copy_out(s, dst, tmp.p, sizeof(double) * s->dim * s->n);
@@ -137,7 +137,7 @@ void dev_free_all(pd_sim *s) {
 extern "C" {
 
 const char *pd_last_error(void) { return g_err.c_str(); }
-const char *pd_version(void) { return "pd-b200 0.2 (sm_100a, FP64, blocked SELL-32xR, warp per R-row group)"; }
+const char *pd_version(void) { return "pd-b200 0.3 (sm_100a, FP64, windowed SELL-32x4, warp per 4-row group)"; }
 
 int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volumes, double horizon,
               const pd_material *mat, const pd_boundary *bc, const pd_runtime *rt) {
@@ -165,11 +165,6 @@ int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volum
   s->s_c = s->fracture ? mat->s_c : 0.0;
   if (rt && rt->alloc && rt->free) { s->rt = *rt; s->own_alloc = false; }
   s->stream = rt ? (cudaStream_t)rt->stream : (cudaStream_t)0;
-  s->R = 4;
-  if (const char *env = getenv("PD_ROWS_PER_THREAD")) {  // tuning knob: 1, 2 or 4 lattice rows per thread
-    int r = atoi(env);
-    if (r == 1 || r == 2 || r == 4) s->R = r;
-  }
   {  // mode constants
     const double nu = mat->nu, kappa = mat->E / (3.0 * (1.0 - 2.0 * nu)), mu = mat->E / (2.0 * (1.0 + nu));
     if (s->mode == PD_MODE_3D) { s->A = 3.0; s->K = 3.0 * kappa; s->G = 15.0 * mu; }
@@ -199,7 +194,7 @@ int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volum
                          (const int32_t *)d_precut, bc ? bc->n_precut : 0);
   if (rc) return fail(rc);
 
-  // ---- state arrays (u, cth live in the node records built above) ----
+  // ---- state arrays (u, cth live in the neighbour records built above) ----
   auto alloc_d = [&](double **p) {
     *p = (double *)pdi::dev_alloc(s, sizeof(double) * s->npad);
     if (*p) cudaMemsetAsync(*p, 0, sizeof(double) * s->npad, s->stream);
@@ -214,11 +209,11 @@ int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volum
   }
   if (!ok) { pdi::set_error("device allocation failed for the state arrays"); return fail(PD_ERR_ALLOC); }
   k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, (const double *)d_u0, s->flags, true,
-                                                         s->rec, PD_F_U(0), nullptr, nullptr, nullptr);
+                                                         s->nb[0], nullptr, nullptr, nullptr);
   k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, (const double *)d_v0, s->flags, true,
-                                                         nullptr, 0, s->v[0], s->v[1], s->v[2]);
+                                                         nullptr, s->v[0], s->v[1], s->v[2]);
   k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, (const double *)d_val, s->flags, false,
-                                                         nullptr, 0, s->bval[0], s->bval[1], s->bval[2]);
+                                                         nullptr, s->bval[0], s->bval[1], s->bval[2]);
   cudaError_t e = cudaGetLastError();
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
   if (e != cudaSuccess) return fail(pdi::cuda_fail(e, "pd_create state initialisation"));
@@ -266,8 +261,8 @@ int pd_step_timed(pd_sim *s, int64_t nsteps, double ms[2]) {
   return rc;
 }
 
-int pd_get_u(pd_sim *s, double *dst) { return s ? get_field(s, dst, PD_F_U(s->cur)) : PD_ERR_ARG; }
-int pd_get_v(pd_sim *s, double *dst) { return s ? get_field(s, dst, -1) : PD_ERR_ARG; }
+int pd_get_u(pd_sim *s, double *dst) { return s ? get_field(s, dst, false) : PD_ERR_ARG; }
+int pd_get_v(pd_sim *s, double *dst) { return s ? get_field(s, dst, true) : PD_ERR_ARG; }
 
 int pd_get_damage(pd_sim *s, double *dst) {
   if (!s || !dst) { pdi::set_error("null argument"); return PD_ERR_ARG; }
@@ -275,7 +270,7 @@ int pd_get_damage(pd_sim *s, double *dst) {
   pdi::launch_damage(s);
   DevTmp tmp(s, sizeof(double) * s->n);
   if (!tmp.p) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
-  k_gather_scalar<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->perm, nullptr, 0, s->phi, (double *)tmp.p);
+  k_gather_scalar<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->perm, s->phi, (double *)tmp.p);
   PD_CUDA(cudaGetLastError());
   return copy_out(s, dst, tmp.p, sizeof(double) * s->n);
 }
@@ -300,14 +295,14 @@ int pd_get_node_fields(pd_sim *s, double *m, double *theta) {
   DevTmp tmp(s, sizeof(double) * s->n), th(s, sizeof(double) * s->npad);
   if (!tmp.p || !th.p) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
   if (m) {
-    k_gather_scalar<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->perm, s->rec, PD_F_M, nullptr, (double *)tmp.p);
+    k_gather_scalar<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->perm, s->m, (double *)tmp.p);
     int rc = copy_out(s, m, tmp.p, sizeof(double) * s->n);
     if (rc) return rc;
   }
   if (theta) {
     flush_break(s);
     pdi::launch_dilatation(s, (double *)th.p, false);
-    k_gather_scalar<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->perm, nullptr, 0, (const double *)th.p, (double *)tmp.p);
+    k_gather_scalar<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->perm, (const double *)th.p, (double *)tmp.p);
     PD_CUDA(cudaGetLastError());
     int rc = copy_out(s, theta, tmp.p, sizeof(double) * s->n);
     if (rc) return rc;

@@ -1,0 +1,131 @@
+// pd_bond.cuh -- the per-bond arithmetic of the two step kernels, shared by the two neighbour-list
+// layouts (pd_step.cu: windowed sliced ELL for any point cloud; pd_lattice.cu: dense lattice tiles).
+//
+//   dilatation (+ break):  dot = xi . eta  [= xbar * e, sqrt-free; rows a1, a2 of SURVEY.md 8(a)]
+//        FRAC: dot - s_c ||xi||^2 >= 0  <=>  e / xbar >= s_c  (Eqs. 1.17, 1.30): the bond breaks
+//        theta_i = (A/m_i) sum_j rho_ij dot V_j           (Eq. 1.6 / 2.3)
+//   force:  f_i = sum_j rho_ij V_j [ cth_i + cth_j + (G/m_i + G/m_j) dot/||xi||^2 ] xi   (Eq. 2.2 / 2.1)
+//
+// Both ends of a bond take the identical break decision because -a*-b == a*b exactly in every
+// product and the sums run in the same component order; every code path (fast / masked, ELL /
+// lattice) uses exactly this arithmetic.
+#pragma once
+#include "pd_internal.cuh"
+
+namespace pdb {
+
+constexpr unsigned FULL = 0xffffffffu;
+
+// one gathered neighbour: DIM pairs {x_k, u_k} (+ {G/m, cth}) (+ V_j)
+template <int DIM, bool AUX, bool VOL>
+struct Ent {
+  double2 p[DIM];
+  double2 g;
+  double vj;
+};
+
+template <int DIM>
+__device__ __forceinline__ double dot3(const double *x, const double *y) {
+  double d = __dmul_rn(x[0], y[0]);
+#pragma unroll
+  for (int k = 1; k < DIM; ++k) d = fma(x[k], y[k], d);
+  return d;
+}
+
+// dilatation (+ break) policy: R rows per lane
+template <int DIM, bool FRAC, bool UNIV, int R>
+struct DilPolicy {
+  using E = Ent<DIM, false, !UNIV>;
+  static constexpr bool kFrac = FRAC;
+  double xo[R][DIM], uo[R][DIM], acc[R], snap[R];
+  double s_c;
+  int sg;   // AND of the sign words of dot - s_c r2 over the fast path's bonds
+
+  __device__ __forceinline__ void fast_begin() {
+    if (FRAC) {
+#pragma unroll
+      for (int r = 0; r < R; ++r) snap[r] = acc[r];
+      sg = (int)0x80000000;
+    }
+  }
+  // true: some bond of the fast pass met the break criterion on some lane; the accumulators are
+  // rolled back and the caller redoes the same bonds with the masked variant
+  __device__ __forceinline__ bool fast_failed() {
+    if (!FRAC) return false;
+    if (!__any_sync(FULL, sg >= 0)) return false;
+#pragma unroll
+    for (int r = 0; r < R; ++r) acc[r] = snap[r];
+    return true;
+  }
+  // returns true if the bond breaks now (MASKED && FRAC only)
+  template <bool MASKED>
+  __device__ __forceinline__ bool bond(int r, const E &e, bool in, bool nofail) {
+    double xi[DIM], eta[DIM];
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) {
+      xi[k] = e.p[k].x - xo[r][k];
+      eta[k] = e.p[k].y - uo[r][k];
+    }
+    const double dot = dot3<DIM>(xi, eta);
+    bool brk = false;
+    if (!MASKED) in = true;
+    if (FRAC) {
+      // s >= s_c breaks (Eq. 1.30): xi.eta - s_c ||xi||^2 >= 0, one rounding, sign read off the high word
+      const double t = fma(-s_c, dot3<DIM>(xi, xi), dot);
+      if (MASKED) {
+        brk = in && __double2hiint(t) >= 0 && !nofail;
+        if (brk) in = false;
+      } else {
+        sg &= __double2hiint(t);
+      }
+    }
+    if (in) {
+      if (UNIV) acc[r] += dot; else acc[r] = fma(e.vj, dot, acc[r]);
+    }
+    return brk;
+  }
+};
+
+// 1/x seed: MUFU.RCP64H (relative error about 2^-20)
+__device__ __forceinline__ double rcp_seed(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  return y;
+}
+
+// force policy
+template <int DIM, bool UNIV, int R>
+struct ForcePolicy {
+  using E = Ent<DIM, true, !UNIV>;
+  static constexpr bool kFrac = false;
+  double xo[R][DIM], uo[R][DIM], f[R][DIM], cth_i[R], gmu_i[R];
+
+  __device__ __forceinline__ void fast_begin() {}
+  __device__ __forceinline__ bool fast_failed() { return false; }
+  template <bool MASKED>
+  __device__ __forceinline__ bool bond(int r, const E &e, bool in, bool) {
+    double xi[DIM], eta[DIM];
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) {
+      xi[k] = e.p[k].x - xo[r][k];
+      eta[k] = e.p[k].y - uo[r][k];
+    }
+    const double dot = dot3<DIM>(xi, eta);
+    const double r2 = dot3<DIM>(xi, xi);
+    // d = dot / r2 = e / xbar: seed y, err = 1 - r2 y, d = dot y (1 + err + err^2)  (relative error err^3 ~ 2^-60)
+    const double y = rcp_seed(r2);
+    const double err = fma(-r2, y, 1.0);
+    const double q = __dmul_rn(dot, y);
+    const double d = fma(q, fma(err, err, err), q);
+    double t = fma(gmu_i[r] + e.g.x, d, cth_i[r] + e.g.y);
+    if (!UNIV) t *= e.vj;
+    if (!MASKED) in = true;   // rho_ij
+    if (in) {
+#pragma unroll
+      for (int k = 0; k < DIM; ++k) f[r][k] = fma(t, xi[k], f[r][k]);
+    }
+    return false;
+  }
+};
+
+}  // namespace pdb

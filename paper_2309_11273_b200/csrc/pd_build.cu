@@ -238,18 +238,23 @@ __global__ void k_final_index(int64_t n, Grid g, const int32_t *__restrict__ row
   iperm[uidx] = fin;
 }
 
-// node records in final order (rec, flags pre-zeroed; phantoms stay zero)
+// node data in final order (arrays pre-zeroed; phantoms stay zero): reference positions into the x half
+// of the position pairs of BOTH neighbour-record buffers, volumes, flags
 __global__ void k_records(int64_t npad, Grid g, const int32_t *__restrict__ perm, const double *__restrict__ coords,
-                          const double *__restrict__ vol, const uint8_t *__restrict__ flags, double *rec,
-                          uint8_t *flagsF) {
+                          const double *__restrict__ vol, const uint8_t *__restrict__ flags, double2 *nb0, double2 *nb1,
+                          double *volF, uint8_t *flagsF) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= npad) return;
   int32_t uidx = perm[i];
   if (uidx < 0) return;
   const int dim = g.dim;
-  double *r = rec + pd_elem(i);
-  for (int k = 0; k < dim; ++k) r[32 * (PD_F_X + k)] = coords[(int64_t)dim * uidx + g.ax[k]];
-  r[32 * PD_F_VOL] = vol[uidx];
+  const uint32_t e = pd_elem(i);
+  for (int k = 0; k < dim; ++k) {
+    const double x = coords[(int64_t)dim * uidx + g.ax[k]];
+    nb0[e + 32 * k].x = x;
+    nb1[e + 32 * k].x = x;
+  }
+  volF[i] = vol[uidx];
   unsigned f = flags ? flags[uidx] : 0u, fi = f & 0xC0u;   // per-dof bits move with their component
   for (int k = 0; k < dim; ++k) {
     if (f & (1u << g.ax[k])) fi |= 1u << k;
@@ -258,24 +263,45 @@ __global__ void k_records(int64_t npad, Grid g, const int32_t *__restrict__ perm
   flagsF[i] = (uint8_t)fi;
 }
 
-// ---- 4./5. lockstep family traversal of one group (one warp; lane = R nodes) -----------------------
-// Calls f(j_final or -1, bits, r2[R]) once per ENTRY, for all 32 lanes together: bits != 0 for the
-// lanes that have a bond to their j there (bit r <=> ||x_j - x_{i_r}||^2 <= h2 and j != i_r).
-template <int R, typename F>
-__device__ __forceinline__ void for_group_family(const Grid &g, int64_t grp, int lane, double h2,
-                                                 const double *__restrict__ rec, const int32_t *__restrict__ perm,
-                                                 const int32_t *__restrict__ cell_start,
-                                                 const int32_t *__restrict__ cell_end,
-                                                 const int32_t *__restrict__ fin1,
-                                                 const int32_t *__restrict__ tile_inv,
-                                                 const int32_t *__restrict__ tile_x0, F f) {
+// ---- 4./5. lockstep family traversal of one group (one warp; lane = 4 nodes) -----------------------
+// The group's neighbourhood is walked COLUMN by column: a column = the cells (cz, bx + dx, *) along
+// internal axis 1 (the axis along which the lane's 4 rows are adjacent).  Per column and lane the
+// bond bits of every cell are found by the exact distance test; then
+//   * if no lane meets a cell with more than one node: SHIFT segments.  With c the cell index along
+//     the column, bond (row r, cell c) belongs to step T = c - r; steps that are a bond for no lane
+//     are dropped, runs of consecutive steps are cut into segments of <= 7 steps, a segment of n
+//     steps lists the n + 3 cells T0 .. T0 + n + 2 as entries (lanes without a node there get
+//     their own node 0 and no bit);
+//   * otherwise FLAT segments: one entry per (cell, k-th node in it) that is a bond for some lane.
+// All lanes of a warp meet the same relative neighbour in the same entry, so the gathers of an
+// entry are contiguous and the segment structure (the CODE nibble) is warp-uniform.
+constexpr int MAXCY = 32;   // cells scanned per column: 4 + 2 S[1] <= 32 (S <= 9 because cell edge >= horizon/8)
+
+struct GroupOut {
+  int ecnt = 0, scnt = 0;
+  int rl[PD_R] = {0, 0, 0, 0};
+  double m[PD_R] = {0, 0, 0, 0}, fv[PD_R] = {0, 0, 0, 0};
+};
+
+template <bool FILL>
+__device__ __forceinline__ void scan_group(const Grid &g, int64_t grp, int lane, double h2,
+                                           const double2 *__restrict__ nb0, const double *__restrict__ vol,
+                                           const int32_t *__restrict__ perm,
+                                           const int32_t *__restrict__ cell_start,
+                                           const int32_t *__restrict__ cell_end,
+                                           const int32_t *__restrict__ fin1,
+                                           const int32_t *__restrict__ tile_inv,
+                                           const int32_t *__restrict__ tile_x0, uint32_t *colp, uint32_t *memp,
+                                           GroupOut &o) {
   constexpr unsigned FULL = 0xffffffffu;
+  constexpr int R = PD_R;
   // nominal cell of the lane
   const int64_t td = tile_inv[grp / g.BZ];
   const int chunk = (int)(td % g.maxchunk);
   const int64_t tr = td / g.maxchunk;
-  const int by0 = (int)(tr % g.ncyg) * g.R, bz = (int)(tr / g.ncyg) * g.BZ + (int)(grp % g.BZ);
+  const int by0 = (int)(tr % g.ncyg) * R, bz = (int)(tr / g.ncyg) * g.BZ + (int)(grp % g.BZ);
   const int bx = tile_x0[tr] + 32 * chunk + lane;
+  const uint32_t self = pd_elem(grp * R * 32 + lane);
   double pi[R][3];
   int64_t ir[R];
   unsigned valid = 0;
@@ -286,179 +312,246 @@ __device__ __forceinline__ void for_group_family(const Grid &g, int64_t grp, int
     pi[r][0] = pi[r][1] = pi[r][2] = 0.0;
     if (perm[ir[r]] >= 0) {
       valid |= 1u << r;
-      const double *p = rec + pd_elem(ir[r]);
-      for (int k = 0; k < g.dim; ++k) pi[r][k] = p[32 * (PD_F_X + k)];
+      const double2 *p = nb0 + pd_elem(ir[r]);
+      for (int k = 0; k < g.dim; ++k) pi[r][k] = p[32 * k].x;
       int q[3];
       cell_of(g, pi[r], q);
       dl = min(dl, q[0] - bx);
       dh = max(dh, q[0] - bx);
     }
   }
-  for (int o = 16; o > 0; o >>= 1) {
-    dl = min(dl, __shfl_xor_sync(FULL, dl, o));
-    dh = max(dh, __shfl_xor_sync(FULL, dh, o));
+  for (int s = 16; s > 0; s >>= 1) {
+    dl = min(dl, __shfl_xor_sync(FULL, dl, s));
+    dh = max(dh, __shfl_xor_sync(FULL, dh, s));
   }
   if (dh < dl) return;  // no node in this group
   const int z0 = g.dim > 2 ? max(bz - g.S[2], 0) : 0, z1 = g.dim > 2 ? min(bz + g.S[2], g.nc[2] - 1) : 0;
-  const int y0 = max(by0 - g.S[1], 0), y1 = min(by0 + g.R - 1 + g.S[1], g.nc[1] - 1);
-  for (int cz = z0; cz <= z1; ++cz)
-    for (int cy = y0; cy <= y1; ++cy) {
-      const int64_t base = ((int64_t)cz * g.nc[1] + cy) * g.nc[0];
-      for (int dx = dl - g.S[0]; dx <= dh + g.S[0]; ++dx) {
-        const int cx = bx + dx;
-        int32_t s = 0, e = 0;
-        if (valid && cx >= 0 && cx < g.nc[0]) { s = cell_start[base + cx]; e = cell_end[base + cx]; }
-        int cnt = e - s, mx = cnt;
-        for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(FULL, mx, o));
-        for (int idx = 0; idx < mx; ++idx) {
-          unsigned bits = 0;
-          double r2[R];
-          int64_t j = -1;
-          if (idx < cnt) {
-            j = fin1[s + idx];
-            const double *q = rec + pd_elem(j);
-            double pj[3] = {0, 0, 0};
-            for (int k = 0; k < g.dim; ++k) pj[k] = q[32 * (PD_F_X + k)];
+  const int y0 = max(by0 - g.S[1], 0), y1 = min(by0 + R - 1 + g.S[1], g.nc[1] - 1);
+  const int ny = min(y1 - y0 + 1, MAXCY);
+
+  auto bond_bits = [&](int64_t j, double *r2) -> unsigned {
+    unsigned bits = 0;
+    const double2 *q = nb0 + pd_elem(j);
+    double pj[3] = {0, 0, 0};
+    for (int k = 0; k < g.dim; ++k) pj[k] = q[32 * k].x;
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-              r2[r] = dist2_exact(g.dim, pi[r], pj);
-              if (((valid >> r) & 1u) && j != ir[r] && r2[r] <= h2) bits |= 1u << r;
-            }
-          }
-          if (__any_sync(FULL, bits != 0)) f(j, bits, r2);
+    for (int r = 0; r < R; ++r) {
+      r2[r] = dist2_exact(g.dim, pi[r], pj);
+      if (((valid >> r) & 1u) && j != ir[r] && r2[r] <= h2) bits |= 1u << r;
+    }
+    return bits;
+  };
+  auto emit_entry = [&](int64_t j) {
+    if (FILL) colp[(int64_t)o.ecnt * 32] = j >= 0 ? pd_elem(j) : self;
+    ++o.ecnt;
+  };
+  auto emit_seg = [&](unsigned code, uint32_t word) {
+    if (FILL) memp[(int64_t)o.scnt * 32] = (code << 28) | word;
+    ++o.scnt;
+  };
+  auto account = [&](int64_t j, unsigned bits, const double *r2) {   // m_i (Eq. 1.9, w = 1), sum_j V_j (Eq. 1.31)
+#pragma unroll
+    for (int r = 0; r < R; ++r) o.rl[r] += (bits >> r) & 1u;
+    if (FILL && bits) {
+      const double vj = vol[j];
+#pragma unroll
+      for (int r = 0; r < R; ++r)
+        if ((bits >> r) & 1u) {
+          o.m[r] = fma(r2[r], vj, o.m[r]);
+          o.fv[r] += vj;
         }
+    }
+  };
+
+  for (int cz = z0; cz <= z1; ++cz)
+    for (int dx = dl - g.S[0]; dx <= dh + g.S[0]; ++dx) {
+      const int cx = bx + dx;
+      const bool inx = valid && cx >= 0 && cx < g.nc[0];
+      // ---- phase 1: bond bits of the first node of every cell of the column ----
+      unsigned char bits[MAXCY];
+      int jj[MAXCY];
+      int maxcnt = 0;
+      unsigned anyb = 0;
+      for (int c = 0; c < ny; ++c) {
+        bits[c] = 0;
+        jj[c] = -1;
+        if (inx) {
+          const int64_t cell = ((int64_t)cz * g.nc[1] + (y0 + c)) * g.nc[0] + cx;
+          const int32_t s = cell_start[cell], cnt = cell_end[cell] - s;
+          maxcnt = max(maxcnt, cnt);
+          if (cnt >= 1) {
+            double r2[R];
+            jj[c] = fin1[s];
+            bits[c] = (unsigned char)bond_bits(jj[c], r2);
+            anyb |= bits[c];
+          }
+        }
+      }
+      if (!__any_sync(FULL, anyb != 0 || maxcnt > 1)) continue;
+      for (int s = 16; s > 0; s >>= 1) maxcnt = max(maxcnt, __shfl_xor_sync(FULL, maxcnt, s));
+      if (maxcnt <= 1) {
+        // ---- SHIFT segments ----
+        int tmin = 1 << 30, tmax = -(1 << 30);
+        for (int c = 0; c < ny; ++c)
+          for (int r = 0; r < R; ++r)
+            if ((bits[c] >> r) & 1u) { tmin = min(tmin, c - r); tmax = max(tmax, c - r); }
+        for (int s = 16; s > 0; s >>= 1) {
+          tmin = min(tmin, __shfl_xor_sync(FULL, tmin, s));
+          tmax = max(tmax, __shfl_xor_sync(FULL, tmax, s));
+        }
+        auto step_bits = [&](int T) -> unsigned {   // bit r: bond (row r, cell T + r)
+          unsigned b = 0;
+          for (int r = 0; r < R; ++r) {
+            const int c = T + r;
+            if (c >= 0 && c < ny && ((bits[c] >> r) & 1u)) b |= 1u << r;
+          }
+          return b;
+        };
+        int T = tmin;
+        while (T <= tmax) {
+          unsigned sb = step_bits(T);
+          if (!__any_sync(FULL, sb != 0)) { ++T; continue; }
+          const int Ta = T;
+          int n = 0;
+          uint32_t word = 0;
+          while (n < PD_MAXSTEP) {
+            word |= sb << (4 * n);
+            ++n;
+            ++T;
+            if (T > tmax) break;
+            sb = step_bits(T);
+            if (!__any_sync(FULL, sb != 0)) break;
+          }
+          for (int c = Ta; c < Ta + n + 3; ++c) emit_entry((c >= 0 && c < ny) ? (int64_t)jj[c] : -1);
+          emit_seg((unsigned)n, word);
+          for (int t = 0; t < n; ++t)
+            for (int r = 0; r < R; ++r)
+              if ((word >> (4 * t + r)) & 1u) {
+                double r2[R];
+                const int64_t j = jj[Ta + t + r];
+                bond_bits(j, r2);
+                account(j, 1u << r, r2);
+              }
+        }
+      } else {
+        // ---- FLAT segments: every (cell, k-th node) that is a bond for some lane ----
+        int n = 0;
+        uint32_t word = 0;
+        for (int c = 0; c < ny; ++c) {
+          int32_t s = 0, cnt = 0;
+          if (inx) {
+            const int64_t cell = ((int64_t)cz * g.nc[1] + (y0 + c)) * g.nc[0] + cx;
+            s = cell_start[cell];
+            cnt = cell_end[cell] - s;
+          }
+          int mx = cnt;
+          for (int q = 16; q > 0; q >>= 1) mx = max(mx, __shfl_xor_sync(FULL, mx, q));
+          for (int idx = 0; idx < mx; ++idx) {
+            unsigned b = 0;
+            double r2[R];
+            int64_t j = -1;
+            if (idx < cnt) { j = fin1[s + idx]; b = bond_bits(j, r2); }
+            if (!__any_sync(FULL, b != 0)) continue;
+            emit_entry(b ? j : -1);
+            account(j, b, r2);
+            word |= b << (4 * n);
+            if (++n == PD_MAXSTEP) { emit_seg(8u + n, word); n = 0; word = 0; }
+          }
+        }
+        if (n) emit_seg(8u + n, word);
       }
     }
 }
 
-template <int R>
-__global__ void k_count(int64_t ngroups, Grid g, double h2, const double *__restrict__ rec,
+__global__ void k_count(int64_t ngroups, Grid g, double h2, const double2 *__restrict__ nb0,
                         const int32_t *__restrict__ perm, const int32_t *__restrict__ cell_start,
                         const int32_t *__restrict__ cell_end, const int32_t *__restrict__ fin1,
                         const int32_t *__restrict__ tile_inv, const int32_t *__restrict__ tile_x0, int32_t *rowlen,
-                        uint32_t *glen) {
+                        uint32_t *glen, uint32_t *slen) {
   int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   int64_t grp = t >> 5;
   if (grp >= ngroups) return;
   int lane = threadIdx.x & 31;
-  int cnt = 0, rl[R];
+  GroupOut o;
+  scan_group<false>(g, grp, lane, h2, nb0, nullptr, perm, cell_start, cell_end, fin1, tile_inv, tile_x0, nullptr, nullptr, o);
 #pragma unroll
-  for (int r = 0; r < R; ++r) rl[r] = 0;
-  for_group_family<R>(g, grp, lane, h2, rec, perm, cell_start, cell_end, fin1, tile_inv, tile_x0,
-                      [&](int64_t, unsigned bits, const double *) {
-                        ++cnt;
-#pragma unroll
-                        for (int r = 0; r < R; ++r) rl[r] += (bits >> r) & 1u;
-                      });
-#pragma unroll
-  for (int r = 0; r < R; ++r) rowlen[(grp * R + r) * 32 + lane] = rl[r];
-  constexpr int EPW = 32 / R;
-  if (lane == 0) glen[grp] = (uint32_t)((cnt + EPW - 1) / EPW * EPW);  // cnt is the same on all lanes
+  for (int r = 0; r < PD_R; ++r) rowlen[(grp * PD_R + r) * 32 + lane] = o.rl[r];
+  if (lane == 0) { glen[grp] = (uint32_t)o.ecnt; slen[grp] = (uint32_t)o.scnt; }  // the same on all lanes
 }
 
-template <int R>
-__global__ void k_fill(int64_t ngroups, Grid g, double h2, double G, double *__restrict__ rec,
-                       const int32_t *__restrict__ perm, const int32_t *__restrict__ cell_start,
-                       const int32_t *__restrict__ cell_end, const int32_t *__restrict__ fin1,
-                       const int32_t *__restrict__ tile_inv, const int32_t *__restrict__ tile_x0,
-                       const uint32_t *__restrict__ goff, uint32_t *col, uint32_t *member) {
+__global__ void k_fill(int64_t ngroups, Grid g, double h2, double G, double2 *__restrict__ nb0, double2 *__restrict__ nb1,
+                       const double *__restrict__ vol, double *__restrict__ mF, double *__restrict__ minvF,
+                       double *__restrict__ fvolF, const int32_t *__restrict__ perm,
+                       const int32_t *__restrict__ cell_start, const int32_t *__restrict__ cell_end,
+                       const int32_t *__restrict__ fin1, const int32_t *__restrict__ tile_inv,
+                       const int32_t *__restrict__ tile_x0, const uint32_t *__restrict__ goff,
+                       const uint32_t *__restrict__ soff, uint32_t *col, uint32_t *member) {
   int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   int64_t grp = t >> 5;
   if (grp >= ngroups) return;
-  constexpr int EPW = 32 / R;
   int lane = threadIdx.x & 31;
-  const int64_t off = goff[grp];
-  const int len = (int)(goff[grp + 1] - goff[grp]);
-  uint32_t *c = col + off * 32 + lane;
-  uint32_t *mb = member + off / EPW * 32 + lane;
-  const uint32_t self = pd_elem(grp * R * 32 + lane);
-  int k = 0;
-  uint32_t word = 0;
-  double m[R], fv[R];
+  GroupOut o;
+  scan_group<true>(g, grp, lane, h2, nb0, vol, perm, cell_start, cell_end, fin1, tile_inv, tile_x0,
+                   col + (int64_t)goff[grp] * 32 + lane, member + (int64_t)soff[grp] * 32 + lane, o);
 #pragma unroll
-  for (int r = 0; r < R; ++r) m[r] = fv[r] = 0.0;
-  for_group_family<R>(g, grp, lane, h2, rec, perm, cell_start, cell_end, fin1, tile_inv, tile_x0,
-                      [&](int64_t j, unsigned bits, const double *r2) {
-                        c[(int64_t)k * 32] = bits ? pd_elem(j) : self;
-                        word |= bits << ((k % EPW) * R);
-                        if (bits) {
-                          double vj = rec[pd_elem(j) + 32 * PD_F_VOL];
-#pragma unroll
-                          for (int r = 0; r < R; ++r)
-                            if ((bits >> r) & 1u) {
-                              m[r] = fma(r2[r], vj, m[r]);  // m_i = sum ||xi||^2 V_j   (Eq. 1.9, w = 1)
-                              fv[r] += vj;                  // sum V_j                   (Eq. 1.31 denominator)
-                            }
-                        }
-                        ++k;
-                        if (k % EPW == 0) { mb[(int64_t)(k / EPW - 1) * 32] = word; word = 0; }
-                      });
-  for (; k < len;) {  // padding entries: own node 0, all bits 0
-    c[(int64_t)k * 32] = self;
-    ++k;
-    if (k % EPW == 0) { mb[(int64_t)(k / EPW - 1) * 32] = word; word = 0; }
-  }
-#pragma unroll
-  for (int r = 0; r < R; ++r) {
-    int64_t i = (grp * R + r) * 32 + lane;
+  for (int r = 0; r < PD_R; ++r) {
+    int64_t i = (grp * PD_R + r) * 32 + lane;
     if (perm[i] < 0) continue;
-    double *p = rec + pd_elem(i);
-    p[32 * PD_F_M] = m[r];
-    p[32 * PD_F_FVOL] = fv[r];
-    p[32 * PD_F_MINV] = m[r] > 0.0 ? 1.0 / m[r] : 0.0;
-    p[32 * PD_F_GMU] = m[r] > 0.0 ? G / m[r] : 0.0;
+    mF[i] = o.m[r];
+    fvolF[i] = o.fv[r];
+    minvF[i] = o.m[r] > 0.0 ? 1.0 / o.m[r] : 0.0;
+    const double gmu = o.m[r] > 0.0 ? G / o.m[r] : 0.0;
+    nb0[pd_elem(i) + 32 * PD_P_AUX].x = gmu;
+    nb1[pd_elem(i) + 32 * PD_P_AUX].x = gmu;
   }
 }
 
 // ---- 6. pre-cuts and no-fail mask ---------------------------------------------------------------
-__global__ void k_precut(int64_t np, int64_t n, int R, const int32_t *__restrict__ pairs,
+__global__ void k_precut(int64_t np, int64_t n, const int32_t *__restrict__ pairs,
                          const int32_t *__restrict__ iperm, const uint32_t *__restrict__ goff,
-                         const uint32_t *__restrict__ col, const uint32_t *__restrict__ member, uint32_t *intact,
-                         unsigned long long *err) {
+                         const uint32_t *__restrict__ soff, const uint32_t *__restrict__ col,
+                         const uint32_t *__restrict__ member, uint32_t *seg, unsigned long long *err) {
   int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= 2 * np) return;
   int64_t pa = pairs[2 * (p >> 1) + (p & 1)], pb = pairs[2 * (p >> 1) + 1 - (p & 1)];
   if (pa < 0 || pa >= n || pb < 0 || pb >= n || pa == pb) { atomicExch(err, 1ull); return; }
   int32_t a = iperm[pa];
   const uint32_t eb = pd_elem(iperm[pb]);
-  const int EPW = 32 / R;
   int64_t slice = a >> 5;
-  int lane = a & 31, r = (int)(slice % R);
-  int64_t grp = slice / R;
-  int64_t off = goff[grp];
-  int len = (int)(goff[grp + 1] - goff[grp]);
-  for (int k = 0; k < len; ++k)
-    if (col[(off + k) * 32 + lane] == eb) {
-      int64_t w = (off + k) / EPW * 32 + lane;
-      uint32_t bit = 1u << ((k % EPW) * R + r);
-      if (member[w] & bit) { atomicAnd(&intact[w], ~bit); return; }
+  int lane = a & 31, ra = (int)(slice % PD_R);
+  int64_t grp = slice / PD_R;
+  const uint32_t *c = col + (int64_t)goff[grp] * 32 + lane;
+  const uint32_t *mb = member + (int64_t)soff[grp] * 32 + lane;
+  uint32_t *sg = seg + (int64_t)soff[grp] * 32 + lane;
+  bool found = false;
+  pd_for_lane_slots(mb, (int)(soff[grp + 1] - soff[grp]), [&](int s, int bit, int r, int k) {
+    if (!found && r == ra && ((mb[(int64_t)s * 32] >> bit) & 1u) && c[(int64_t)k * 32] == eb) {
+      atomicAnd(&sg[(int64_t)s * 32], ~(1u << bit));
+      found = true;
     }
-  atomicExch(err, 1ull);  // not a bond
+  });
+  if (!found) atomicExch(err, 1ull);  // not a bond
 }
 
-__global__ void k_nofail(int64_t ngroups, int R, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ goff,
-                         const uint32_t *__restrict__ col, const uint32_t *__restrict__ member, uint32_t *nofail) {
+__global__ void k_nofail(int64_t ngroups, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ goff,
+                         const uint32_t *__restrict__ soff, const uint32_t *__restrict__ col,
+                         const uint32_t *__restrict__ member, uint32_t *nofail) {
   int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   int64_t grp = t >> 5;
   if (grp >= ngroups) return;
   int lane = threadIdx.x & 31;
-  const int EPW = 32 / R;
-  int64_t off = goff[grp];
-  int len = (int)(goff[grp + 1] - goff[grp]);
+  const int nseg = (int)(soff[grp + 1] - soff[grp]);
+  const uint32_t *c = col + (int64_t)goff[grp] * 32 + lane;
+  const uint32_t *mb = member + (int64_t)soff[grp] * 32 + lane;
+  uint32_t *nf = nofail + (int64_t)soff[grp] * 32 + lane;
   unsigned fi = 0;  // bit r: node r is no-fail
-  for (int r = 0; r < R; ++r)
-    if (flags[(grp * R + r) * 32 + lane] & PD_NO_FAIL) fi |= 1u << r;
-  const unsigned all = (1u << R) - 1u;
-  for (int w = 0; w * EPW < len; ++w) {
-    uint32_t word = 0;
-    for (int q = 0; q < EPW; ++q) {
-      int64_t j = pd_elem_inv(col[(off + w * EPW + q) * 32 + lane]);
-      unsigned nf = (flags[j] & PD_NO_FAIL) ? all : fi;
-      word |= nf << (q * R);
-    }
-    int64_t wi = (off / EPW + w) * 32 + lane;
-    nofail[wi] = word & member[wi];
-  }
+  for (int r = 0; r < PD_R; ++r)
+    if (flags[(grp * PD_R + r) * 32 + lane] & PD_NO_FAIL) fi |= 1u << r;
+  for (int s = 0; s < nseg; ++s) nf[(int64_t)s * 32] = mb[(int64_t)s * 32] & 0xf0000000u;
+  pd_for_lane_slots(mb, nseg, [&](int s, int bit, int r, int k) {
+    if (!((mb[(int64_t)s * 32] >> bit) & 1u)) return;
+    if (((fi >> r) & 1u) || (flags[pd_elem_inv(c[(int64_t)k * 32])] & PD_NO_FAIL)) nf[(int64_t)s * 32] |= 1u << bit;
+  });
 }
 
 __global__ void k_checks(int64_t npad, const int32_t *__restrict__ perm, const int32_t *__restrict__ rowlen,
@@ -478,31 +571,30 @@ __global__ void k_rowlen_user(int64_t n, const int32_t *__restrict__ iperm, cons
   out[uidx] = rowlen[iperm[uidx]];
 }
 
-__global__ void k_export_rows(int64_t ngroups, int R, const int32_t *__restrict__ perm,
+__global__ void k_export_rows(int64_t ngroups, const int32_t *__restrict__ perm,
                               const long long *__restrict__ rowptr, const uint32_t *__restrict__ goff,
-                              const uint32_t *__restrict__ col, const uint32_t *__restrict__ member,
-                              const uint32_t *__restrict__ intact, int32_t *col_out, uint8_t *intact_out) {
+                              const uint32_t *__restrict__ soff, const uint32_t *__restrict__ col,
+                              const uint32_t *__restrict__ member, const uint32_t *__restrict__ seg,
+                              int32_t *col_out, uint8_t *intact_out) {
   int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   int64_t grp = t >> 5;
   if (grp >= ngroups) return;
   int lane = threadIdx.x & 31;
-  const int EPW = 32 / R;
-  int64_t off = goff[grp];
-  int len = (int)(goff[grp + 1] - goff[grp]);
-  for (int r = 0; r < R; ++r) {
-    int32_t uidx = perm[(grp * R + r) * 32 + lane];
-    if (uidx < 0) continue;
-    long long base = rowptr[uidx];
-    for (int k = 0; k < len; ++k) {
-      int64_t w = (off + k) / EPW * 32 + lane;
-      uint32_t bit = 1u << ((k % EPW) * R + r);
-      if (member[w] & bit) {
-        col_out[base] = perm[pd_elem_inv(col[(off + k) * 32 + lane])];
-        intact_out[base] = (intact[w] & bit) ? 1 : 0;
-        ++base;
-      }
-    }
+  const int nseg = (int)(soff[grp + 1] - soff[grp]);
+  const uint32_t *c = col + (int64_t)goff[grp] * 32 + lane;
+  const uint32_t *mb = member + (int64_t)soff[grp] * 32 + lane;
+  const uint32_t *sg = seg + (int64_t)soff[grp] * 32 + lane;
+  long long base[PD_R];
+  for (int r = 0; r < PD_R; ++r) {
+    int32_t uidx = perm[(grp * PD_R + r) * 32 + lane];
+    base[r] = uidx >= 0 ? rowptr[uidx] : -1;
   }
+  pd_for_lane_slots(mb, nseg, [&](int s, int bit, int r, int k) {
+    if (base[r] < 0 || !((mb[(int64_t)s * 32] >> bit) & 1u)) return;
+    col_out[base[r]] = perm[pd_elem_inv(c[(int64_t)k * 32])];
+    intact_out[base[r]] = (uint8_t)((sg[(int64_t)s * 32] >> bit) & 1u);
+    ++base[r];
+  });
 }
 
 inline unsigned nblk(int64_t n) { return (unsigned)((n + TPB - 1) / TPB); }
@@ -533,8 +625,7 @@ int build_family(pd_sim *s, const double *coords, const double *vol, const uint8
   cudaStream_t st = s->stream;
   const int64_t n = s->n;
   const int dim = s->dim;
-  const int R = s->R;
-  const int EPW = 32 / R;
+  const int R = PD_R;
 
   // ---- scratch (freed at the end through the same allocator) ----
   std::vector<void *> scratch;
@@ -702,7 +793,7 @@ int build_family(pd_sim *s, const double *coords, const double *vol, const uint8
   s->ngroups = (int64_t)ntile * g.BZ;
   s->nslices = s->ngroups * R;
   s->npad = s->nslices * 32;
-  if (s->npad >= (1ll << 31) - 64 || s->npad * PD_NF >= (1ll << 32)) { set_error("too many nodes after padding"); return PD_ERR_LIMIT; }
+  if (s->npad >= (1ll << 31) - 64 || s->npad * PD_NP >= (1ll << 32)) { set_error("too many nodes after padding"); return PD_ERR_LIMIT; }
 
   SCRATCH(fin1, int32_t, n);
   SCRATCH(tile_inv, int32_t, ntile);
@@ -711,30 +802,40 @@ int build_family(pd_sim *s, const double *coords, const double *vol, const uint8
   PD_CUDA(cudaMemsetAsync(s->perm, 0xff, sizeof(int32_t) * s->npad, st));
   k_final_index<<<nblk(n), TPB, 0, st>>>(n, g, rowid, vx, ord1, tile_ord, tile_inv, fin1, s->perm, s->iperm);
 
-  BUILD_ALLOC(s->rec, double, s->npad * PD_NF);
+  for (int q = 0; q < 2; ++q) {
+    BUILD_ALLOC(s->nb[q], double2, s->npad * PD_NP);
+    PD_CUDA(cudaMemsetAsync(s->nb[q], 0, sizeof(double2) * s->npad * PD_NP, st));
+  }
+  BUILD_ALLOC(s->vol, double, s->npad);
+  BUILD_ALLOC(s->m, double, s->npad);
+  BUILD_ALLOC(s->minv, double, s->npad);
+  BUILD_ALLOC(s->fvol, double, s->npad);
   BUILD_ALLOC(s->flags, uint8_t, s->npad);
-  PD_CUDA(cudaMemsetAsync(s->rec, 0, sizeof(double) * s->npad * PD_NF, st));
+  for (double *p : {s->vol, s->m, s->minv, s->fvol}) PD_CUDA(cudaMemsetAsync(p, 0, sizeof(double) * s->npad, st));
   PD_CUDA(cudaMemsetAsync(s->flags, 0, s->npad, st));
-  k_records<<<nblk(s->npad), TPB, 0, st>>>(s->npad, g, s->perm, coords, vol, flags, s->rec, s->flags);
+  k_records<<<nblk(s->npad), TPB, 0, st>>>(s->npad, g, s->perm, coords, vol, flags, s->nb[0], s->nb[1], s->vol, s->flags);
 
   // ---- 4. count -> group lengths -> offsets ----
   const double h2 = s->horizon * s->horizon;
   BUILD_ALLOC(s->rowlen, int32_t, s->npad);
   BUILD_ALLOC(s->goff, uint32_t, s->ngroups + 1);
+  BUILD_ALLOC(s->soff, uint32_t, s->ngroups + 1);
   SCRATCH(glen, uint32_t, s->ngroups + 1);
+  SCRATCH(slen, uint32_t, s->ngroups + 1);
   PD_CUDA(cudaMemsetAsync(glen + s->ngroups, 0, sizeof(uint32_t), st));
+  PD_CUDA(cudaMemsetAsync(slen + s->ngroups, 0, sizeof(uint32_t), st));
   const unsigned gblk = nblk(s->ngroups * 32);
-  switch (R) {
-    case 1: k_count<1><<<gblk, TPB, 0, st>>>(s->ngroups, g, h2, s->rec, s->perm, cell_start, cell_end, fin1, tile_inv, tile_x0, s->rowlen, glen); break;
-    case 2: k_count<2><<<gblk, TPB, 0, st>>>(s->ngroups, g, h2, s->rec, s->perm, cell_start, cell_end, fin1, tile_inv, tile_x0, s->rowlen, glen); break;
-    default: k_count<4><<<gblk, TPB, 0, st>>>(s->ngroups, g, h2, s->rec, s->perm, cell_start, cell_end, fin1, tile_inv, tile_x0, s->rowlen, glen); break;
-  }
+  k_count<<<gblk, TPB, 0, st>>>(s->ngroups, g, h2, s->nb[0], s->perm, cell_start, cell_end, fin1, tile_inv, tile_x0,
+                                s->rowlen, glen, slen);
   {
     int rc = scan_exclusive<uint32_t>(s, scratch, glen, s->goff, s->ngroups + 1);
     if (rc) return rc;
+    rc = scan_exclusive<uint32_t>(s, scratch, slen, s->soff, s->ngroups + 1);
+    if (rc) return rc;
   }
-  uint32_t total_entries = 0;
+  uint32_t total_entries = 0, total_segs = 0;
   PD_CUDA(cudaMemcpyAsync(&total_entries, s->goff + s->ngroups, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+  PD_CUDA(cudaMemcpyAsync(&total_segs, s->soff + s->ngroups, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
   SCRATCH(zsum, long long, 1);
   {
     cub::TransformInputIterator<long long, cub::CastOp<long long>, const int32_t *> it(s->rowlen, cub::CastOp<long long>());
@@ -752,37 +853,42 @@ int build_family(pd_sim *s, const double *coords, const double *vol, const uint8
   PD_CUDA(cudaStreamSynchronize(st));
   s->Z = hz;
   s->nentries = total_entries;
+  s->nsegs = total_segs;
   if (hred[0]) { set_error("a node has an empty family (m_i = 0); enlarge the horizon"); return PD_ERR_ISOLATED; }
   if (s->Z >= (1ll << 31)) {
     set_error("more than 2^31 directed bonds");
+    return PD_ERR_LIMIT;
+  }
+  if ((uint64_t)total_entries * 32 >= (1ull << 32) - 32 * (PD_COL_SLACK + 1)) {
+    set_error("neighbour list too long for 32-bit offsets");
     return PD_ERR_LIMIT;
   }
   s->has_nofail = (hred[1] & 1ull) != 0;
   s->has_bc = (hred[1] & 2ull) != 0;
 
   // ---- 5. fill ----
-  const size_t nwords = (size_t)(total_entries / EPW) * 32;
-  BUILD_ALLOC(s->col, uint32_t, (size_t)total_entries * 32 + 32);
-  BUILD_ALLOC(s->member, uint32_t, nwords + 32);
-  BUILD_ALLOC(s->intact, uint32_t, nwords + 32);
-  switch (R) {
-    case 1: k_fill<1><<<gblk, TPB, 0, st>>>(s->ngroups, g, h2, s->G, s->rec, s->perm, cell_start, cell_end, fin1, tile_inv, tile_x0, s->goff, s->col, s->member); break;
-    case 2: k_fill<2><<<gblk, TPB, 0, st>>>(s->ngroups, g, h2, s->G, s->rec, s->perm, cell_start, cell_end, fin1, tile_inv, tile_x0, s->goff, s->col, s->member); break;
-    default: k_fill<4><<<gblk, TPB, 0, st>>>(s->ngroups, g, h2, s->G, s->rec, s->perm, cell_start, cell_end, fin1, tile_inv, tile_x0, s->goff, s->col, s->member); break;
-  }
-  PD_CUDA(cudaMemcpyAsync(s->intact, s->member, sizeof(uint32_t) * nwords, cudaMemcpyDeviceToDevice, st));
+  const size_t ncol = ((size_t)total_entries + PD_COL_SLACK) * 32, nwords = ((size_t)total_segs + 8) * 32;
+  BUILD_ALLOC(s->col, uint32_t, ncol);
+  BUILD_ALLOC(s->member, uint32_t, nwords);
+  BUILD_ALLOC(s->seg, uint32_t, nwords);
+  PD_CUDA(cudaMemsetAsync(s->col + (size_t)total_entries * 32, 0, sizeof(uint32_t) * 32 * PD_COL_SLACK, st));  // slack: node 0
+  PD_CUDA(cudaMemsetAsync(s->member + (size_t)total_segs * 32, 0, sizeof(uint32_t) * 8 * 32, st));
+  k_fill<<<gblk, TPB, 0, st>>>(s->ngroups, g, h2, s->G, s->nb[0], s->nb[1], s->vol, s->m, s->minv, s->fvol, s->perm,
+                               cell_start, cell_end, fin1, tile_inv, tile_x0, s->goff, s->soff, s->col, s->member);
+  PD_CUDA(cudaMemcpyAsync(s->seg, s->member, sizeof(uint32_t) * nwords, cudaMemcpyDeviceToDevice, st));
 
   // ---- 6. pre-cuts, no-fail ----
   if (n_precut > 0) {
     PD_CUDA(cudaMemsetAsync(red, 0, sizeof(unsigned long long), st));
-    k_precut<<<nblk(2 * n_precut), TPB, 0, st>>>(n_precut, n, R, precut, s->iperm, s->goff, s->col, s->member, s->intact, red);
+    k_precut<<<nblk(2 * n_precut), TPB, 0, st>>>(n_precut, n, precut, s->iperm, s->goff, s->soff, s->col, s->member, s->seg, red);
     PD_CUDA(cudaMemcpyAsync(hred, red, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     PD_CUDA(cudaStreamSynchronize(st));
     if (hred[0]) { set_error("a pre-cut pair is out of range or not a bond"); return PD_ERR_ARG; }
   }
   if (s->has_nofail && s->fracture) {
-    BUILD_ALLOC(s->nofail, uint32_t, nwords + 32);
-    k_nofail<<<gblk, TPB, 0, st>>>(s->ngroups, R, s->flags, s->goff, s->col, s->member, s->nofail);
+    BUILD_ALLOC(s->nofail, uint32_t, nwords);
+    PD_CUDA(cudaMemsetAsync(s->nofail, 0, sizeof(uint32_t) * nwords, st));
+    k_nofail<<<gblk, TPB, 0, st>>>(s->ngroups, s->flags, s->goff, s->soff, s->col, s->member, s->nofail);
   }
   PD_CUDA(cudaGetLastError());
   PD_CUDA(cudaStreamSynchronize(st));
@@ -806,8 +912,8 @@ int export_bond_mask(pd_sim *s, long long *rowptr_dev, int32_t *col_dev, uint8_t
     if (!tmp) { set_error("device allocation failed"); rc = PD_ERR_ALLOC; break; }
     if (cub::DeviceScan::ExclusiveSum(tmp, tb, cnt, rowptr_dev, (int)(n + 1), st) != cudaSuccess) { rc = PD_ERR_CUDA; break; }
     if (col_dev && intact_dev)
-      k_export_rows<<<nblk(s->ngroups * 32), TPB, 0, st>>>(s->ngroups, s->R, s->perm, rowptr_dev, s->goff, s->col,
-                                                            s->member, s->intact, col_dev, intact_dev);
+      k_export_rows<<<nblk(s->ngroups * 32), TPB, 0, st>>>(s->ngroups, s->perm, rowptr_dev, s->goff, s->soff, s->col,
+                                                            s->member, s->seg, col_dev, intact_dev);
     if (cudaGetLastError() != cudaSuccess) rc = PD_ERR_CUDA;
   } while (0);
   cudaStreamSynchronize(st);

@@ -1,29 +1,36 @@
 // pd_internal.cuh -- private state of libpd.so (not part of the boundary; see include/pd.h).
 //
 // Data layout in HBM.  Nodes are renumbered by the builder into a
-// FINAL order made of 32-node SLICES (one warp lane per node); R consecutive slices form a
-// GROUP (one warp): lane l of group g owns the R nodes (g*R + r)*32 + l, r = 0..R-1, which the
-// builder chooses to be the l-th nodes of R adjacent lattice rows.  Missing nodes are PHANTOMS
-// (perm = -1, zero record, no bonds).
+// FINAL order made of 32-node SLICES (one warp lane per node); PD_R = 4 consecutive slices form a
+// GROUP (one warp): lane l of group g owns the 4 nodes (g*4 + r)*32 + l, r = 0..3, which the
+// builder chooses to be the l-th nodes of 4 lattice rows adjacent along internal axis 1.
+// Missing nodes are PHANTOMS (perm = -1, zero records, no bonds).
+// Vector components are stored in INTERNAL order: component k = user component ax[k]; internal
+// axis 0 is the lane axis chosen by the builder.
 //
-//   rec : node records, AoSoA-32 with PD_NF = 16 FP64 fields per node:
-//         element index elem(i) = (i >> 5) * (32*PD_NF) + (i & 31); field f lives at elem + 32 f
-//         (so a warp reads 256 contiguous bytes per field and one address serves all fields).
-//         (vector components are stored in INTERNAL order: component k = user component ax[k],
-//          internal axis 0 = the lane axis chosen by the builder)
-//         fields: 0-2 x (reference position)   3 gmu = G/m_i      4 vol = V_i     5 minv = 1/m_i
-//                 6 m_i                        7 fvol = sum_j V_j
-//                 8-10 u (buffer 0)  11 cth (buffer 0)   12-14 u (buffer 1)  15 cth (buffer 1)
-//         cth_i = (K - G/3) theta_i / m_i belongs to the u buffer it was computed from.
-//   blocked sliced ELL ("SELL-32xR"): group g has glen[g] ENTRIES starting at goff[g]; entry k of
-//         lane l is ONE neighbour shared by the lane's R nodes:
-//           col   [(goff[g] + k)*32 + l]            elem() of the neighbour
-//           intact[(goff[g] + k)/EPW*32 + l]        bit ((k % EPW)*R + r): bond (node r, neighbour)
-//                                                   exists and is unbroken (Eq. 1.30); EPW = 32/R
-//           member[...]  same shape, static: the bond exists (family membership)
-//           nofail[...]  same shape, static, only if some node is no-fail
-//         padding entries point at the lane's own node 0 and have all bits 0.
+//   nb[b], b = 0, 1 : NEIGHBOUR RECORDS, the data a bond gathers from its far end, as 16-byte pairs
+//         in AoSoA-32: pair p of node i sits at double2 index  pd_elem(i) + 32 p,
+//         pd_elem(i) = (i >> 5) * (32 * PD_NP) + (i & 31), so a warp reads 512 contiguous bytes per
+//         pair with one LDG.128 per lane.
+//           pair k < 3 : { x_k (reference position, static), u_k }      (buffer b holds u^n for cur = b)
+//           pair 3     : { G/m_i (static),  cth_i = (K - G/3) theta_i / m_i of the u in this buffer }
+//   own-node statics (SoA [npad]): vol = V_i, minv = 1/m_i, m = m_i, fvol = sum_j V_j
 //   v, bval : SoA [dim][npad];  flags, rowlen, phi : [npad]
+//
+//   neighbour lists ("windowed SELL-32x4"): group g owns the ENTRIES goff[g] .. goff[g+1]-1 and the
+//   SEGMENTS soff[g] .. soff[g+1]-1.
+//     col[(goff[g] + k)*32 + l]   = pd_elem() of the node lane l gathers in entry k (own node 0 if none)
+//     seg[(soff[g] + s)*32 + l]   = one 32-bit word per lane and segment:
+//           bits 28-31  CODE, the same on all 32 lanes:
+//                 1..7   SHIFT segment of n = CODE steps over n + 3 consecutive entries: in step t
+//                        row r pairs with entry t + r (a window sliding along the rows' axis: the
+//                        4 rows are adjacent lattice rows, so entry t + r is the same RELATIVE
+//                        neighbour for every row; one gathered neighbour serves up to 4 bonds)
+//                 9..15  FLAT segment of n = CODE - 8 steps over n entries: in step t all rows pair
+//                        with entry t (general point clouds, cells holding several nodes)
+//                 0      padding (skipped)
+//           bits 0-27   bit 4 t + r : the bond (row r, step t) exists and is unbroken (Eq. 1.30)
+//     member / nofail : same shape as seg, static: the bond exists / may never break
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -34,31 +41,49 @@
 #include "../../include/pd.h"
 
 #define PD_MAX_DIM 3
-#define PD_NF 16          // FP64 fields per node record
-#define PD_F_X 0
-#define PD_F_GMU 3
-#define PD_F_VOL 4
-#define PD_F_MINV 5
-#define PD_F_M 6
-#define PD_F_FVOL 7
-#define PD_F_U(buf) (8 + 4 * (buf))
-#define PD_F_CTH(buf) (11 + 4 * (buf))
-#define PD_GROUPS_PER_CTA 4   // 128 threads; in 3D the 4 groups of a CTA are 4 z-levels of one tile
+#define PD_R 4            // rows (nodes) per lane
+#define PD_NP 4           // 16-byte pairs per node in a neighbour record
+#define PD_P_AUX 3        // pair {G/m, cth}
+#define PD_MAXSTEP 7      // steps per segment (28 mask bits)
+#define PD_GROUPS_PER_CTA 4   // 128 threads; in 3D the 4 groups of a CTA are 4 levels (internal axis 2) of one tile
+#define PD_COL_SLACK 64   // readable entries past the end of col (the kernels prefetch indices ahead)
 
 __host__ __device__ __forceinline__ uint32_t pd_elem(int64_t i) {
-  return (uint32_t)((i >> 5) * (32 * PD_NF) + (i & 31));
+  return (uint32_t)((i >> 5) * (32 * PD_NP) + (i & 31));
 }
 __host__ __device__ __forceinline__ int64_t pd_elem_inv(uint32_t e) {
-  return ((int64_t)(e / (32 * PD_NF)) << 5) | (e & 31);
+  return ((int64_t)(e / (32 * PD_NP)) << 5) | (e & 31);
+}
+
+// Calls f(s, bit, r, k) for every bond slot of one lane: s = segment index inside the group,
+// bit = 4 t + r, k = entry index inside the group.  `words` = the lane's segment words (any of
+// seg / member / nofail: only the CODE nibble is read here), stride 32.
+template <typename F>
+__host__ __device__ __forceinline__ void pd_for_lane_slots(const uint32_t *words, int nseg, F f) {
+  int e = 0;
+  for (int s = 0; s < nseg; ++s) {
+    const uint32_t code = words[(int64_t)s * 32] >> 28;
+    if (code == 0) continue;
+    if (code < 8) {
+      const int n = (int)code;
+      for (int t = 0; t < n; ++t)
+        for (int r = 0; r < PD_R; ++r) f(s, 4 * t + r, r, e + t + r);
+      e += n + 3;
+    } else {
+      const int n = (int)code - 8;
+      for (int t = 0; t < n; ++t)
+        for (int r = 0; r < PD_R; ++r) f(s, 4 * t + r, r, e + t);
+      e += n;
+    }
+  }
 }
 
 struct pd_sim {
   // scalars
   int dim = 0, mode = 0;
-  int R = 4;                    // rows (nodes) per thread
   int ax[3] = {0, 1, 2};        // internal component k = user component ax[k]; internal 0 is the lane axis
   int64_t n = 0, npad = 0, nslices = 0, ngroups = 0;
-  int64_t Z = 0, nentries = 0;  // directed bonds; stored entries per lane (sum of glen)
+  int64_t Z = 0, nentries = 0, nsegs = 0;  // directed bonds; stored entries / segments per lane
   double horizon = 0, A = 0, K = 0, G = 0, c1 = 0;  // c1 = K - G/3
   double rho = 0, dt = 0, s_c = 0, ramp_time = 0, vol_uniform = 0;
   bool fracture = false, uniform_v = false, has_nofail = false, has_bc = false;
@@ -71,17 +96,18 @@ struct pd_sim {
   size_t bytes_held = 0;
   // node arrays (final order)
   int32_t *perm = nullptr, *iperm = nullptr;  // perm[final] = user or -1, iperm[user] = final
-  double *rec = nullptr;
+  double2 *nb[2] = {nullptr, nullptr};
+  double *vol = nullptr, *minv = nullptr, *m = nullptr, *fvol = nullptr;
   double *v[PD_MAX_DIM] = {}, *bval[PD_MAX_DIM] = {};
   double *phi = nullptr;
   uint8_t *flags = nullptr;
   int32_t *rowlen = nullptr;
-  // blocked SELL
-  uint32_t *goff = nullptr;   // [ngroups + 1] entry offsets (multiples of EPW)
+  // windowed SELL
+  uint32_t *goff = nullptr, *soff = nullptr;   // [ngroups + 1] entry / segment offsets
   uint32_t *col = nullptr;
-  uint32_t *intact = nullptr, *member = nullptr, *nofail = nullptr;
+  uint32_t *seg = nullptr, *member = nullptr, *nofail = nullptr;
   // state
-  int cur = 0;            // which u buffer holds u^n
+  int cur = 0;            // which buffer holds u^n
   int64_t step = 0;       // n
   int64_t launches = 0;   // kernels launched by pd_step
   bool break_pending = false;  // u^n has not been break-checked yet (deferred step 5)

@@ -1,44 +1,51 @@
 // pd_step.cu -- the per-step kernels.
 //
-// One warp per GROUP of the blocked sliced-ELL layout (pd_internal.cuh): lane l owns R nodes (the
-// l-th nodes of R adjacent lattice rows) and walks the lane's entry list.  An entry is one
-// neighbour j; x_j, u_j (and G/m_j, cth_j) are gathered ONCE and serve the up-to-R bonds
-// (i_r, j), r = 0..R-1, whose bits are set -- register blocking of the gather, which is what
-// the L1 data pipe, the index stream and the instruction issue are all short of (profiles/).
-// In the bulk of a lattice body the 32 lanes of a warp see the same relative neighbour in entry
-// k, so every gather of a warp is 256 contiguous bytes per field, and which (entry, r) pairs
-// are bonds is warp-uniform: pairs that are a bond for no lane are skipped with a uniform
-// branch (the OR of the mask word over the warp, one REDUX per word).
+// One warp per GROUP of the windowed sliced-ELL layout (pd_internal.cuh): lane l owns 4 nodes (the
+// l-th nodes of 4 adjacent lattice rows) and walks the group's SEGMENTS.  A SHIFT segment of n
+// steps covers n + 3 consecutive entries of one lattice column; in step t row r pairs with entry
+// t + r, so the four bonds of a step are the SAME relative neighbour for the four rows: a window of
+// 4 gathered neighbour records slides along the column in registers, one new record per step
+// serves 4 bonds (register blocking of the gather), the four bonds of a step are independent
+// FP64 chains in one basic block (ILP 4), and -- when every lane has all 4 n bonds of the
+// segment intact, the normal case in the bulk -- there is not a single mask test or branch per
+// bond (FAST path).  Segments with missing / broken bonds on some lane run the MASKED variant
+// (predicated accumulation, steps that are empty for the whole warp skipped).
 //
 //   k_dilatation  (rows a1, a2, and a5's break test folded in):
 //        for each intact bond  dot = xi . eta            [= xbar * e, sqrt-free]
-//        FRAC: if dot >= s_c * ||xi||^2 (<=> e/xbar >= s_c, Eq. 1.17/1.30) clear the bit first
+//        FRAC: a bond with dot - s_c ||xi||^2 >= 0 (<=> e/xbar >= s_c, Eq. 1.17/1.30) breaks first.
+//              The fast path only ANDs the sign words of these values; if any of them is
+//              non-negative on any lane the segment is redone by the masked variant, which
+//              clears the bits.
 //        theta_i = (A/m_i) sum_j rho_ij dot V_j           (Eq. 1.6 / 2.3)
-//        writes cth_i = (K - G/3) theta_i / m_i
+//        writes the pair { G/m_i, cth_i = (K - G/3) theta_i / m_i }
 //   k_force_update (rows a1, a3, a4):
 //        f_i = sum_j rho_ij V_j [ cth_i + cth_j + (G/m_i + G/m_j) dot/||xi||^2 ] xi   (Eq. 2.2 / 2.1)
-//        then Eq. 2.11 + boundary dofs, u^{n+1} into the other u buffer
+//        then Eq. 2.11 + boundary dofs, {x, u^{n+1}} into the other neighbour-record buffer
 //   k_damage (row a5): phi_i (Eq. 1.31) + device-side reduction of the three damage scalars
 //
 // The break test of step n (on u^{n+1}) runs at the start of step n+1's dilatation pass, which
 // needs the same xi . eta; pd_api.cu flushes it before any state is read back.  Both ends of a
 // bond take the identical decision because -a*-b == a*b exactly in every product and the sums
-// run in the same component order.
-#include "pd_internal.cuh"
+// run in the same component order; fast and masked variants use the same arithmetic.
+#include "pd_bond.cuh"
 
 namespace {
 
+using pdb::Ent;
+
 constexpr int TPB = 32 * PD_GROUPS_PER_CTA;
-constexpr unsigned FULL = 0xffffffffu;
-constexpr int EB = 8;   // entries per pipelined block (a whole mask word when R = 4)
+using pdb::FULL;
+constexpr int NCQ = PD_MAXSTEP + 3;   // entries of the longest segment
 
 struct StepArgs {
   int64_t ngroups;
-  double *rec;
-  const uint32_t *goff;
-  const uint32_t *col;
-  uint32_t *intact;
-  const uint32_t *nofail;
+  const double2 *nbr;   // neighbour records holding u^n (and, for the force pass, cth^n)
+  double2 *nbw;         // dilatation: the same buffer (pair AUX is written); force: the other buffer
+  const uint32_t *goff, *soff, *col;
+  uint32_t *seg;
+  const uint32_t *member, *nofail;
+  const double *vol, *minv, *fvol;
   double *v[3];
   const double *bval[3];
   double *theta_out;
@@ -47,251 +54,215 @@ struct StepArgs {
   const int32_t *rowlen;
   const int32_t *perm;
   unsigned long long *stats;
-  double A, c1, s_c, vol_uniform, rho, dt, ramp_time;
+  double A, c1, G, s_c, vol_uniform, rho, dt, ramp_time;
   int64_t step;
 };
 
-// 1/x to ~1 ulp: hardware seed (MUFU.RCP64H, rel. err 2^-23) + one cubic Newton step:
-// y (1 + e + e^2) with e = 1 - x y  leaves (1/x)(1 - e^3).
-__device__ __forceinline__ double rcp_fast(double x) {
-  double y;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double e = fma(-x, y, 1.0);
-  double t = fma(e, e, e);
-  return fma(y, t, y);
-}
-
-template <int DIM>
-__device__ __forceinline__ double dot_xi_eta(const double *xi, const double *eta) {
-  double d = xi[0] * eta[0];
+template <int DIM, bool AUX, bool VOL>
+__device__ __forceinline__ void load_ent(Ent<DIM, AUX, VOL> &E, const StepArgs &a, uint32_t c) {
+  const double2 *q = a.nbr + c;
 #pragma unroll
-  for (int k = 1; k < DIM; ++k) d = fma(xi[k], eta[k], d);
-  return d;
+  for (int k = 0; k < DIM; ++k) E.p[k] = __ldg(q + 32 * k);
+  if (AUX) E.g = __ldg(q + 32 * PD_P_AUX);
+  if (VOL) E.vj = __ldg(a.vol + (((c >> 7) << 5) | (c & 31)));
 }
 
 // ---------------------------------------------------------------------------------------------
-template <int DIM, int R, bool FRAC, bool UNIV, int CUR>
-__global__ void __launch_bounds__(TPB) k_dilatation(StepArgs a) {
-  constexpr int EPW = 32 / R;
-  constexpr uint32_t RMASK = (1u << R) - 1u;
-  constexpr uint32_t BMASK = EB * R == 32 ? 0xffffffffu : ((1u << (EB * R)) - 1u);
-  const int lane = threadIdx.x & 31;
-  const int64_t grp = ((int64_t)blockIdx.x * TPB + threadIdx.x) >> 5;
-  if (grp >= a.ngroups) return;
-  double *rec = a.rec;
-  const uint32_t e0 = pd_elem(grp * R * 32 + lane);
+// predicated 16-byte read-only load: no branch, so the four bonds of a step stay in one basic block
+__device__ __forceinline__ void ldg_if(double2 &v, const double2 *ptr, uint32_t pred) {
+  asm("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %3, 0;\n\t@p ld.global.nc.v2.f64 {%0, %1}, [%2];\n\t}"
+      : "+d"(v.x), "+d"(v.y) : "l"(ptr), "r"(pred));
+}
+template <int DIM, bool AUX, bool VOL>
+__device__ __forceinline__ void load_ent_if(Ent<DIM, AUX, VOL> &E, const StepArgs &a, uint32_t c, uint32_t pred) {
+  const double2 *q = a.nbr + c;
+#pragma unroll
+  for (int k = 0; k < DIM; ++k) ldg_if(E.p[k], q + 32 * k, pred);
+  if (AUX) ldg_if(E.g, q + 32 * PD_P_AUX, pred);
+  if (VOL) { if (pred) E.vj = __ldg(a.vol + (((c >> 7) << 5) | (c & 31))); }
+}
 
-  double xi_[R][DIM], ui_[R][DIM], acc[R];
+// one SHIFT segment: n steps over the entries cc[0 .. n+2].  The window S[4] lives across segments:
+// in step t row r uses S[(t + r) % 4]; the slot of row 0 is refilled with entry t + 4 as soon as
+// row 0 is done.  In the LAST step every slot dies as its row finishes and is refilled with one of
+// the first four entries of the NEXT segment (cq[0..3], slot j <- cq[j]), so the next segment
+// finds its window already in flight (`preloaded`).
+template <bool MASKED, class P>
+__device__ __forceinline__ void run_shift(P &p, const StepArgs &a, int n, uint32_t mask, uint32_t nf, uint32_t &clr,
+                                          const uint32_t (&cc)[NCQ], const uint32_t (&cq)[NCQ], typename P::E (&S)[4],
+                                          bool preloaded) {
+  if (!preloaded) {
 #pragma unroll
-  for (int r = 0; r < R; ++r) {
-    acc[r] = 0.0;
+    for (int q = 0; q < 4; ++q) load_ent(S[q], a, cc[q]);
+  }
+  uint32_t anyw = 0;
+  if (MASKED) anyw = __reduce_or_sync(FULL, mask);
+  auto bond = [&](int r, const typename P::E &e, int bit) {
+    if (p.template bond<MASKED>(r, e, (mask >> bit) & 1u, (nf >> bit) & 1u)) clr |= 1u << bit;
+  };
 #pragma unroll
-    for (int k = 0; k < DIM; ++k) {
-      xi_[r][k] = rec[e0 + r * 32 * PD_NF + 32 * (PD_F_X + k)];
-      ui_[r][k] = rec[e0 + r * 32 * PD_NF + 32 * (PD_F_U(CUR) + k)];
+  for (int t = 0; t < PD_MAXSTEP; ++t) {
+    if (t < n) {
+      const uint32_t last = (t + 1 == n) ? 1u : 0u;                    // warp-uniform
+      const bool live = !MASKED || ((anyw >> (4 * t)) & 15u) != 0;   // warp-uniform
+      if (live) bond(0, S[t % 4], 4 * t + 0);
+      load_ent(S[t % 4], a, last ? cq[t % 4] : cc[(t + 4) % NCQ]);
+      if (live) bond(1, S[(t + 1) % 4], 4 * t + 1);
+      load_ent_if(S[(t + 1) % 4], a, cq[(t + 1) % 4], last);
+      if (live) bond(2, S[(t + 2) % 4], 4 * t + 2);
+      load_ent_if(S[(t + 2) % 4], a, cq[(t + 2) % 4], last);
+      if (live) bond(3, S[(t + 3) % 4], 4 * t + 3);
+      load_ent_if(S[(t + 3) % 4], a, cq[(t + 3) % 4], last);
     }
   }
-  const uint32_t off = a.goff[grp];
-  const uint32_t nwords = (a.goff[grp + 1] - off) / EPW;
-  const uint32_t *col = a.col + (int64_t)off * 32 + lane;
-  uint32_t *bits = a.intact + (int64_t)(off / EPW) * 32 + lane;
-  const uint32_t *nofail = (FRAC && a.nofail) ? a.nofail + (int64_t)(off / EPW) * 32 + lane : nullptr;
+}
 
-  // entries are walked in blocks of EB = 8: the 8 neighbour indices of the NEXT block are loaded
-  // before the current block is processed, and the node data of entry q+1 before entry q is used
-  // (software pipeline in registers; the index stream comes from HBM, the node data from L1/L2).
-  const uint32_t nblocks = nwords * (EPW / EB);
-  uint32_t cn[EB], mwn = 0;
-  if (nblocks) {
+constexpr int PF_AHEAD = 24;   // entries
+constexpr int PF_SEG = 4;      // segments
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
+// walks all segments of the warp's group
+template <class P>
+__device__ __forceinline__ void walk_group(P &p, const StepArgs &a, int64_t grp, int lane) {
+  const uint32_t s0 = a.soff[grp], nseg = a.soff[grp + 1] - s0;
+  const uint32_t *colp = a.col + (int64_t)a.goff[grp] * 32 + lane;
+  const int64_t wbase = (int64_t)s0 * 32 + lane;
+  // the segment word and the NCQ neighbour indices of the NEXT segment are loaded while the current
+  // one is processed (the index stream comes from HBM; the node data from L1/L2)
+  uint32_t wn = 0, cq[NCQ];
+  prefetch_l2(colp + (int64_t)(NCQ + lane) * 32 - lane);
+  if (lane < PF_SEG) prefetch_l2(a.seg + wbase - lane + (int64_t)lane * 32);
+  if (nseg) wn = a.seg[wbase];
 #pragma unroll
-    for (int q = 0; q < EB; ++q) cn[q] = col[q * 32];
-    mwn = bits[0];
-  }
-  for (uint32_t blk = 0; blk < nblocks; ++blk) {
-    const uint32_t w = blk / (EPW / EB), sh = (blk % (EPW / EB)) * (EB * R);
-    uint32_t c[EB];
+  for (int q = 0; q < NCQ; ++q) cq[q] = colp[q * 32];
+  uint32_t e = 0;
+  typename P::E S[4];
+  bool pre = false;   // S already holds (in flight) the first four entries of the segment about to start
+  for (uint32_t s = 0; s < nseg; ++s) {
+    const uint32_t w = wn;
+    uint32_t cc[NCQ];
 #pragma unroll
-    for (int q = 0; q < EB; ++q) c[q] = cn[q];
-    uint32_t mwfull = (EPW == EB) ? mwn : bits[w * 32];
-    if (blk + 1 < nblocks) {
+    for (int q = 0; q < NCQ; ++q) cc[q] = cq[q];
+    const uint32_t code = w >> 28;
+    const uint32_t nent = code == 0 ? 0u : (code < 8 ? code + 3 : code - 8);
+    const uint32_t en = e + nent;
+    if (s + 1 < nseg) wn = a.seg[wbase + (int64_t)(s + 1) * 32];
+    // the index and mask streams are read once, line by line, straight from HBM: pull the lines of the
+    // entries PF_AHEAD .. PF_AHEAD + nent - 1 past the next segment (one line per lane) and of the
+    // segment word PF_SEG ahead into L2, so the loads above find them there
+    if ((uint32_t)lane < nent) prefetch_l2(colp + (int64_t)(en + PF_AHEAD + lane) * 32 - lane);
+    if (lane == 0 && s + PF_SEG < nseg) prefetch_l2(a.seg + wbase + (int64_t)(s + PF_SEG) * 32);
 #pragma unroll
-      for (int q = 0; q < EB; ++q) cn[q] = col[((blk + 1) * EB + q) * 32];
-      if (EPW == EB) mwn = bits[(w + 1) * 32];
-    }
-    uint32_t mw = (mwfull >> sh) & BMASK;
-    const uint32_t anyw = __reduce_or_sync(FULL, mw);   // warp-uniform: pairs that are a bond for some lane
-    if (anyw == 0) continue;
-    const uint32_t mw0 = mw;
-    uint32_t nf = 0;
-    if (FRAC && nofail) nf = (nofail[w * 32] >> sh) & BMASK;
-    double xj[DIM], uj[DIM], vj = 0.0, xn[DIM], un[DIM], vn = 0.0;
-    {
-      const double *p = rec + c[0];
-#pragma unroll
-      for (int k = 0; k < DIM; ++k) { xn[k] = __ldg(p + 32 * (PD_F_X + k)); un[k] = __ldg(p + 32 * (PD_F_U(CUR) + k)); }
-      if (!UNIV) vn = __ldg(p + 32 * PD_F_VOL);
-    }
-#pragma unroll
-    for (int q = 0; q < EB; ++q) {
-#pragma unroll
-      for (int k = 0; k < DIM; ++k) { xj[k] = xn[k]; uj[k] = un[k]; }
-      vj = vn;
-      if (q + 1 < EB) {
-        const double *p = rec + c[q + 1];
-#pragma unroll
-        for (int k = 0; k < DIM; ++k) { xn[k] = __ldg(p + 32 * (PD_F_X + k)); un[k] = __ldg(p + 32 * (PD_F_U(CUR) + k)); }
-        if (!UNIV) vn = __ldg(p + 32 * PD_F_VOL);
+    for (int q = 0; q < NCQ; ++q) cq[q] = colp[(int64_t)(en + q) * 32];   // col has PD_COL_SLACK readable entries past its end
+    const uint32_t mask = w & 0x0fffffffu;
+    if (code >= 1 && code < 8) {
+      const int n = (int)code;
+      const uint32_t fullmask = (1u << (4 * n)) - 1u;
+      bool slow = !__all_sync(FULL, mask == fullmask);
+      uint32_t clr = 0;
+      if (!slow) {
+        p.fast_begin();
+        run_shift<false>(p, a, n, mask, 0u, clr, cc, cq, S, pre);
+        slow = p.fast_failed();
+        pre = false;   // (only matters if the segment is redone: the window now holds the next segment's entries)
       }
-      if (((anyw >> (q * R)) & RMASK) == 0) continue;
+      if (slow) {
+        const uint32_t nf = (P::kFrac && a.nofail) ? a.nofail[wbase + (int64_t)s * 32] : 0u;
+        run_shift<true>(p, a, n, mask, nf, clr, cc, cq, S, pre);
+        if (clr) a.seg[wbase + (int64_t)s * 32] = w & ~clr;
+      }
+      pre = true;
+    } else if (code > 8) {
+      pre = false;
+      const int n = (int)code - 8;
+      const uint32_t nf = (P::kFrac && a.nofail) ? a.nofail[wbase + (int64_t)s * 32] : 0u;
+      uint32_t clr = 0;
+#pragma unroll 1
+      for (int t = 0; t < n; ++t) {
+        typename P::E S1;
+        load_ent(S1, a, colp[(int64_t)(e + t) * 32]);
 #pragma unroll
-      for (int r = 0; r < R; ++r) {
-        const uint32_t bit = 1u << (q * R + r);
-        if (anyw & bit) {
-          double xi[DIM], eta[DIM];
-#pragma unroll
-          for (int k = 0; k < DIM; ++k) {
-            xi[k] = xj[k] - xi_[r][k];
-            eta[k] = uj[k] - ui_[r][k];
-          }
-          const double dot = dot_xi_eta<DIM>(xi, eta);
-          const bool in = (mw & bit) != 0;
-          bool brk = false;
-          if (FRAC) {
-            // s >= s_c breaks (Eq. 1.30): xi.eta - s_c ||xi||^2 >= 0, one rounding, sign read off the high word
-            const double t = fma(-a.s_c, dot_xi_eta<DIM>(xi, xi), dot);
-            brk = in && __double2hiint(t) >= 0 && !(nf & bit);
-            if (brk) mw ^= bit;
-          }
-          if (in && !brk) {
-            if (UNIV) acc[r] += dot; else acc[r] = fma(vj, dot, acc[r]);
-          }
+        for (int r = 0; r < PD_R; ++r) {
+          const int bit = 4 * t + r;
+          if (p.template bond<true>(r, S1, (mask >> bit) & 1u, (nf >> bit) & 1u)) clr |= 1u << bit;
         }
       }
+      if (clr) a.seg[wbase + (int64_t)s * 32] = w & ~clr;
     }
-    if (FRAC && mw != mw0) bits[w * 32] = mwfull & ~((mw0 & ~mw) << sh);
-  }
-#pragma unroll
-  for (int r = 0; r < R; ++r) {
-    const uint32_t e = e0 + r * 32 * PD_NF;
-    if (UNIV) acc[r] *= a.vol_uniform;
-    const double mi = rec[e + 32 * PD_F_MINV];   // 0 for phantoms
-    const double theta = a.A * mi * acc[r];
-    rec[e + 32 * PD_F_CTH(CUR)] = a.c1 * theta * mi;
-    if (a.theta_out) a.theta_out[(grp * R + r) * 32 + lane] = theta;
+    e = en;
   }
 }
 
 // ---------------------------------------------------------------------------------------------
-template <int DIM, int R, bool UNIV, int CUR>
-__global__ void __launch_bounds__(TPB) k_force_update(StepArgs a) {
-  constexpr int EPW = 32 / R;
-  constexpr uint32_t RMASK = (1u << R) - 1u;
-  constexpr uint32_t BMASK = EB * R == 32 ? 0xffffffffu : ((1u << (EB * R)) - 1u);
+template <int DIM, bool FRAC, bool UNIV>
+__global__ void __launch_bounds__(TPB, 3) k_dilatation(StepArgs a) {
   const int lane = threadIdx.x & 31;
   const int64_t grp = ((int64_t)blockIdx.x * TPB + threadIdx.x) >> 5;
   if (grp >= a.ngroups) return;
-  double *rec = a.rec;
-  const uint32_t e0 = pd_elem(grp * R * 32 + lane);
-
-  double xi_[R][DIM], ui_[R][DIM], f[R][DIM], cth_i[R], gmu_i[R];
+  const uint32_t e0 = pd_elem(grp * PD_R * 32 + lane);
+  pdb::DilPolicy<DIM, FRAC, UNIV, PD_R> p;
+  p.s_c = a.s_c;
 #pragma unroll
-  for (int r = 0; r < R; ++r) {
-    const uint32_t e = e0 + r * 32 * PD_NF;
+  for (int r = 0; r < PD_R; ++r) {
+    p.acc[r] = 0.0;
 #pragma unroll
     for (int k = 0; k < DIM; ++k) {
-      xi_[r][k] = rec[e + 32 * (PD_F_X + k)];
-      ui_[r][k] = rec[e + 32 * (PD_F_U(CUR) + k)];
-      f[r][k] = 0.0;
+      const double2 xu = a.nbr[e0 + r * 32 * PD_NP + 32 * k];
+      p.xo[r][k] = xu.x;
+      p.uo[r][k] = xu.y;
     }
-    cth_i[r] = rec[e + 32 * PD_F_CTH(CUR)];
-    gmu_i[r] = rec[e + 32 * PD_F_GMU];
   }
-  const uint32_t off = a.goff[grp];
-  const uint32_t nwords = (a.goff[grp + 1] - off) / EPW;
-  const uint32_t *col = a.col + (int64_t)off * 32 + lane;
-  const uint32_t *bits = a.intact + (int64_t)(off / EPW) * 32 + lane;
+  walk_group(p, a, grp, lane);
+#pragma unroll
+  for (int r = 0; r < PD_R; ++r) {
+    const int64_t i = (grp * PD_R + r) * 32 + lane;
+    double s = p.acc[r];
+    if (UNIV) s *= a.vol_uniform;
+    const double mi = a.minv[i];   // 0 for phantoms
+    const double theta = a.A * mi * s;
+    a.nbw[e0 + r * 32 * PD_NP + 32 * PD_P_AUX] = make_double2(a.G * mi, a.c1 * theta * mi);
+    if (a.theta_out) a.theta_out[i] = theta;
+  }
+}
 
-  const uint32_t nblocks = nwords * (EPW / EB);
-  uint32_t cn[EB], mwn = 0;
-  if (nblocks) {
+// ---------------------------------------------------------------------------------------------
+template <int DIM, bool UNIV>
+__global__ void __launch_bounds__(TPB, 2) k_force_update(StepArgs a) {
+  const int lane = threadIdx.x & 31;
+  const int64_t grp = ((int64_t)blockIdx.x * TPB + threadIdx.x) >> 5;
+  if (grp >= a.ngroups) return;
+  const uint32_t e0 = pd_elem(grp * PD_R * 32 + lane);
+  pdb::ForcePolicy<DIM, UNIV, PD_R> p;
 #pragma unroll
-    for (int q = 0; q < EB; ++q) cn[q] = col[q * 32];
-    mwn = bits[0];
+  for (int r = 0; r < PD_R; ++r) {
+    const uint32_t e = e0 + r * 32 * PD_NP;
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) {
+      const double2 xu = a.nbr[e + 32 * k];
+      p.xo[r][k] = xu.x;
+      p.uo[r][k] = xu.y;
+      p.f[r][k] = 0.0;
+    }
+    const double2 g = a.nbr[e + 32 * PD_P_AUX];
+    p.gmu_i[r] = g.x;
+    p.cth_i[r] = g.y;
   }
-  for (uint32_t blk = 0; blk < nblocks; ++blk) {
-    const uint32_t w = blk / (EPW / EB), sh = (blk % (EPW / EB)) * (EB * R);
-    uint32_t c[EB];
-#pragma unroll
-    for (int q = 0; q < EB; ++q) c[q] = cn[q];
-    const uint32_t mwfull = (EPW == EB) ? mwn : bits[w * 32];
-    if (blk + 1 < nblocks) {
-#pragma unroll
-      for (int q = 0; q < EB; ++q) cn[q] = col[((blk + 1) * EB + q) * 32];
-      if (EPW == EB) mwn = bits[(w + 1) * 32];
-    }
-    const uint32_t mw = (mwfull >> sh) & BMASK;
-    const uint32_t anyw = __reduce_or_sync(FULL, mw);
-    if (anyw == 0) continue;
-    double xj[DIM], uj[DIM], gj, cj, vj = 0.0, xn[DIM], un[DIM], gn, cnx, vn = 0.0;
-    {
-      const double *p = rec + c[0];
-#pragma unroll
-      for (int k = 0; k < DIM; ++k) { xn[k] = __ldg(p + 32 * (PD_F_X + k)); un[k] = __ldg(p + 32 * (PD_F_U(CUR) + k)); }
-      gn = __ldg(p + 32 * PD_F_GMU);
-      cnx = __ldg(p + 32 * PD_F_CTH(CUR));
-      if (!UNIV) vn = __ldg(p + 32 * PD_F_VOL);
-    }
-#pragma unroll
-    for (int q = 0; q < EB; ++q) {
-#pragma unroll
-      for (int k = 0; k < DIM; ++k) { xj[k] = xn[k]; uj[k] = un[k]; }
-      gj = gn; cj = cnx; vj = vn;
-      if (q + 1 < EB) {
-        const double *p = rec + c[q + 1];
-#pragma unroll
-        for (int k = 0; k < DIM; ++k) { xn[k] = __ldg(p + 32 * (PD_F_X + k)); un[k] = __ldg(p + 32 * (PD_F_U(CUR) + k)); }
-        gn = __ldg(p + 32 * PD_F_GMU);
-        cnx = __ldg(p + 32 * PD_F_CTH(CUR));
-        if (!UNIV) vn = __ldg(p + 32 * PD_F_VOL);
-      }
-      if (((anyw >> (q * R)) & RMASK) == 0) continue;
-#pragma unroll
-      for (int r = 0; r < R; ++r) {
-        const uint32_t bit = 1u << (q * R + r);
-        if (anyw & bit) {
-          double xi[DIM], eta[DIM];
-#pragma unroll
-          for (int k = 0; k < DIM; ++k) {
-            xi[k] = xj[k] - xi_[r][k];
-            eta[k] = uj[k] - ui_[r][k];
-          }
-          const double dot = dot_xi_eta<DIM>(xi, eta);
-          const double r2 = dot_xi_eta<DIM>(xi, xi);
-          const double d = dot * rcp_fast(r2);                       // e / xbar
-          double t = fma(gmu_i[r] + gj, d, cth_i[r] + cj);
-          if (!UNIV) t *= vj;
-          t = (mw & bit) ? t : 0.0;                                  // rho_ij
-#pragma unroll
-          for (int k = 0; k < DIM; ++k) f[r][k] = fma(t, xi[k], f[r][k]);
-        }
-      }
-    }
-  }
+  walk_group(p, a, grp, lane);
   // ---- Eq. 2.11 + boundary dofs (App. B) ----
   double g = 1.0;
   if (a.ramp_time > 0.0) g = fmin(1.0, __ddiv_rn(__dmul_rn((double)a.step, a.dt), a.ramp_time));
 #pragma unroll
-  for (int r = 0; r < R; ++r) {
-    const int64_t i = (grp * R + r) * 32 + lane;
+  for (int r = 0; r < PD_R; ++r) {
+    const int64_t i = (grp * PD_R + r) * 32 + lane;
     if (a.perm[i] < 0) continue;   // phantom
-    const uint32_t e = e0 + r * 32 * PD_NF;
+    const uint32_t e = e0 + r * 32 * PD_NP;
     const unsigned fl = a.flags[i];
 #pragma unroll
     for (int k = 0; k < DIM; ++k) {
-      double fk = f[r][k];
+      double fk = p.f[r][k];
       if (UNIV) fk *= a.vol_uniform;
       double vk = a.v[k][i];
-      double uk = ui_[r][k];
+      double uk = p.uo[r][k];
       if (fl & (1u << k)) {                       // clamped: u stays, v = 0
         vk = 0.0;
       } else if (fl & (8u << k)) {                // prescribed velocity
@@ -304,49 +275,52 @@ __global__ void __launch_bounds__(TPB) k_force_update(StepArgs a) {
         uk = __dadd_rn(uk, __dmul_rn(a.dt, vk));
       }
       a.v[k][i] = vk;
-      rec[e + 32 * (PD_F_U(CUR ^ 1) + k)] = uk;
+      a.nbw[e + 32 * k] = make_double2(p.xo[r][k], uk);
     }
   }
 }
 
 // ---------------------------------------------------------------------------------------------
 // phi_i = 1 - sum_j rho_ij V_j / sum_j V_j (Eq. 1.31) and the three damage scalars.
-template <int R>
 __global__ void __launch_bounds__(TPB) k_damage(StepArgs a, bool univ) {
-  constexpr int EPW = 32 / R;
   const int lane = threadIdx.x & 31;
   const int64_t grp = ((int64_t)blockIdx.x * TPB + threadIdx.x) >> 5;
   unsigned long long broken = 0, ge_half = 0;
   double phimax = 0.0;
   if (grp < a.ngroups) {
-    const double *rec = a.rec;
-    const uint32_t off = a.goff[grp];
-    const uint32_t nwords = (a.goff[grp + 1] - off) / EPW;
-    const uint32_t *col = a.col + (int64_t)off * 32 + lane;
-    const uint32_t *bits = a.intact + (int64_t)(off / EPW) * 32 + lane;
-    double sum[R];
-    int cnt[R];
+    const uint32_t s0 = a.soff[grp];
+    const int nseg = (int)(a.soff[grp + 1] - s0);
+    const uint32_t *sg = a.seg + (int64_t)s0 * 32 + lane;
+    const uint32_t *mb = a.member + (int64_t)s0 * 32 + lane;
+    const uint32_t *col = a.col + (int64_t)a.goff[grp] * 32 + lane;
+    double sum[PD_R];
+    int cnt[PD_R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) { sum[r] = 0.0; cnt[r] = 0; }
-    for (uint32_t w = 0; w < nwords; ++w) {
-      const uint32_t mw = bits[w * 32];
-      if (mw == 0) continue;
-      for (int q = 0; q < EPW; ++q) {
-        const uint32_t nib = (mw >> (q * R)) & ((R == 32) ? 0xffffffffu : ((1u << R) - 1u));
-        if (!nib) continue;
-        double vj = a.vol_uniform;
-        if (!univ) vj = rec[col[(w * EPW + q) * 32] + 32 * PD_F_VOL];
+    for (int r = 0; r < PD_R; ++r) { sum[r] = 0.0; cnt[r] = 0; }
+    if (univ) {
+      for (int s = 0; s < nseg; ++s) {
+        const uint32_t w = sg[(int64_t)s * 32] & 0x0fffffffu;
 #pragma unroll
-        for (int r = 0; r < R; ++r)
-          if ((nib >> r) & 1u) { sum[r] += vj; ++cnt[r]; }
+        for (int r = 0; r < PD_R; ++r) cnt[r] += __popc(w & (0x01111111u << r));
       }
+#pragma unroll
+      for (int r = 0; r < PD_R; ++r)   // the sum of cnt equal volumes, added one by one like sum_j V_j was (pd_build.cu)
+        for (int q = 0; q < cnt[r]; ++q) sum[r] += a.vol_uniform;
+    } else {
+      pd_for_lane_slots(mb, nseg, [&](int s, int bit, int r, int k) {
+        if (!((sg[(int64_t)s * 32] >> bit) & 1u)) return;
+        const uint32_t c = col[(int64_t)k * 32];
+        const double vj = a.vol[((c >> 7) << 5) | (c & 31)];
+#pragma unroll
+        for (int q = 0; q < PD_R; ++q)
+          if (q == r) { sum[q] += vj; ++cnt[q]; }
+      });
     }
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-      const int64_t i = (grp * R + r) * 32 + lane;
+    for (int r = 0; r < PD_R; ++r) {
+      const int64_t i = (grp * PD_R + r) * 32 + lane;
       if (a.perm[i] < 0) continue;
-      const double fvol = rec[pd_elem(i) + 32 * PD_F_FVOL];
-      const double phi = 1.0 - sum[r] / fvol;
+      const double phi = 1.0 - sum[r] / a.fvol[i];
       a.phi[i] = phi;
       broken += (unsigned long long)(a.rowlen[i] - cnt[r]);
       ge_half += phi >= 0.5 ? 1ull : 0ull;
@@ -371,31 +345,27 @@ __global__ void __launch_bounds__(TPB) k_damage(StepArgs a, bool univ) {
 StepArgs make_args(pd_sim *s) {
   StepArgs a{};
   a.ngroups = s->ngroups;
-  a.rec = s->rec; a.goff = s->goff; a.col = s->col; a.intact = s->intact; a.nofail = s->nofail;
+  a.nbr = s->nb[s->cur]; a.nbw = s->nb[s->cur];
+  a.goff = s->goff; a.soff = s->soff; a.col = s->col; a.seg = s->seg; a.member = s->member; a.nofail = s->nofail;
+  a.vol = s->vol; a.minv = s->minv; a.fvol = s->fvol;
   for (int k = 0; k < 3; ++k) { a.v[k] = s->v[k]; a.bval[k] = s->bval[k]; }
   a.theta_out = nullptr; a.phi = s->phi; a.flags = s->flags; a.rowlen = s->rowlen; a.perm = s->perm;
   a.stats = s->stats_dev;
-  a.A = s->A; a.c1 = s->c1; a.s_c = s->s_c; a.vol_uniform = s->vol_uniform; a.rho = s->rho; a.dt = s->dt;
+  a.A = s->A; a.c1 = s->c1; a.G = s->G; a.s_c = s->s_c; a.vol_uniform = s->vol_uniform; a.rho = s->rho; a.dt = s->dt;
   a.ramp_time = s->ramp_time; a.step = s->step;
   return a;
 }
 
 inline unsigned ngrid(const pd_sim *s) { return (unsigned)((s->ngroups + PD_GROUPS_PER_CTA - 1) / PD_GROUPS_PER_CTA); }
 
-template <int DIM, int R, bool FRAC, bool UNIV>
-void dil_cur(const StepArgs &a, int cur, unsigned grid, cudaStream_t st) {
-  if (cur) k_dilatation<DIM, R, FRAC, UNIV, 1><<<grid, TPB, 0, st>>>(a);
-  else k_dilatation<DIM, R, FRAC, UNIV, 0><<<grid, TPB, 0, st>>>(a);
+template <int DIM>
+void dil_dispatch(const StepArgs &a, bool frac, bool univ, unsigned grid, cudaStream_t st) {
+  if (frac) { if (univ) k_dilatation<DIM, true, true><<<grid, TPB, 0, st>>>(a); else k_dilatation<DIM, true, false><<<grid, TPB, 0, st>>>(a); }
+  else { if (univ) k_dilatation<DIM, false, true><<<grid, TPB, 0, st>>>(a); else k_dilatation<DIM, false, false><<<grid, TPB, 0, st>>>(a); }
 }
-template <int DIM, int R>
-void dil_dispatch(const StepArgs &a, bool frac, bool univ, int cur, unsigned grid, cudaStream_t st) {
-  if (frac) { if (univ) dil_cur<DIM, R, true, true>(a, cur, grid, st); else dil_cur<DIM, R, true, false>(a, cur, grid, st); }
-  else { if (univ) dil_cur<DIM, R, false, true>(a, cur, grid, st); else dil_cur<DIM, R, false, false>(a, cur, grid, st); }
-}
-template <int DIM, int R>
-void force_dispatch(const StepArgs &a, bool univ, int cur, unsigned grid, cudaStream_t st) {
-  if (univ) { if (cur) k_force_update<DIM, R, true, 1><<<grid, TPB, 0, st>>>(a); else k_force_update<DIM, R, true, 0><<<grid, TPB, 0, st>>>(a); }
-  else { if (cur) k_force_update<DIM, R, false, 1><<<grid, TPB, 0, st>>>(a); else k_force_update<DIM, R, false, 0><<<grid, TPB, 0, st>>>(a); }
+template <int DIM>
+void force_dispatch(const StepArgs &a, bool univ, unsigned grid, cudaStream_t st) {
+  if (univ) k_force_update<DIM, true><<<grid, TPB, 0, st>>>(a); else k_force_update<DIM, false><<<grid, TPB, 0, st>>>(a);
 }
 
 }  // namespace
@@ -406,41 +376,23 @@ int launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
   StepArgs a = make_args(s);
   a.theta_out = theta_out;
   const bool frac = do_break && s->fracture;
-  const unsigned grid = ngrid(s);
-  if (s->dim == 2) {
-    if (s->R == 1) dil_dispatch<2, 1>(a, frac, s->uniform_v, s->cur, grid, s->stream);
-    else if (s->R == 2) dil_dispatch<2, 2>(a, frac, s->uniform_v, s->cur, grid, s->stream);
-    else dil_dispatch<2, 4>(a, frac, s->uniform_v, s->cur, grid, s->stream);
-  } else {
-    if (s->R == 1) dil_dispatch<3, 1>(a, frac, s->uniform_v, s->cur, grid, s->stream);
-    else if (s->R == 2) dil_dispatch<3, 2>(a, frac, s->uniform_v, s->cur, grid, s->stream);
-    else dil_dispatch<3, 4>(a, frac, s->uniform_v, s->cur, grid, s->stream);
-  }
+  if (s->dim == 2) dil_dispatch<2>(a, frac, s->uniform_v, ngrid(s), s->stream);
+  else dil_dispatch<3>(a, frac, s->uniform_v, ngrid(s), s->stream);
   return PD_OK;
 }
 
 int launch_force_update(pd_sim *s) {
   StepArgs a = make_args(s);
-  const unsigned grid = ngrid(s);
-  if (s->dim == 2) {
-    if (s->R == 1) force_dispatch<2, 1>(a, s->uniform_v, s->cur, grid, s->stream);
-    else if (s->R == 2) force_dispatch<2, 2>(a, s->uniform_v, s->cur, grid, s->stream);
-    else force_dispatch<2, 4>(a, s->uniform_v, s->cur, grid, s->stream);
-  } else {
-    if (s->R == 1) force_dispatch<3, 1>(a, s->uniform_v, s->cur, grid, s->stream);
-    else if (s->R == 2) force_dispatch<3, 2>(a, s->uniform_v, s->cur, grid, s->stream);
-    else force_dispatch<3, 4>(a, s->uniform_v, s->cur, grid, s->stream);
-  }
+  a.nbw = s->nb[s->cur ^ 1];
+  if (s->dim == 2) force_dispatch<2>(a, s->uniform_v, ngrid(s), s->stream);
+  else force_dispatch<3>(a, s->uniform_v, ngrid(s), s->stream);
   return PD_OK;
 }
 
 int launch_damage(pd_sim *s) {
   StepArgs a = make_args(s);
   cudaMemsetAsync(s->stats_dev, 0, 3 * sizeof(unsigned long long), s->stream);
-  const unsigned grid = ngrid(s);
-  if (s->R == 1) k_damage<1><<<grid, TPB, 0, s->stream>>>(a, s->uniform_v);
-  else if (s->R == 2) k_damage<2><<<grid, TPB, 0, s->stream>>>(a, s->uniform_v);
-  else k_damage<4><<<grid, TPB, 0, s->stream>>>(a, s->uniform_v);
+  k_damage<<<ngrid(s), TPB, 0, s->stream>>>(a, s->uniform_v);
   return PD_OK;
 }
 
