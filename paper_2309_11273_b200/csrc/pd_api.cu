@@ -17,7 +17,7 @@ inline unsigned nblk(int64_t n) { return (unsigned)((n + TPB - 1) / TPB); }
 // buffer (nb != NULL) or SoA arrays
 struct Ax { int a[3]; };
 __global__ void k_scatter_field(int64_t npad, int dim, Ax ax, const int32_t *__restrict__ perm, const double *__restrict__ src,
-                                const uint8_t *__restrict__ flags, bool clamp_zero, double2 *nb, double *d0,
+                                const uint8_t *__restrict__ flags, bool clamp_zero, double2 *nb, bool lattice, double *d0,
                                 double *d1, double *d2) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= npad) return;
@@ -27,12 +27,12 @@ __global__ void k_scatter_field(int64_t npad, int dim, Ax ax, const int32_t *__r
   for (int k = 0; k < dim; ++k) {
     double val = (src && uidx >= 0) ? src[(int64_t)dim * uidx + ax.a[k]] : 0.0;
     if (clamp_zero && (fl & (1u << k))) val = 0.0;
-    if (nb) nb[pd_elem(i) + 32 * k].y = val; else d[k][i] = val;
+    if (nb) nb[pd_pair_index(lattice, npad, i, k)].y = val; else d[k][i] = val;
   }
 }
 
 // final order -> user AoS; source is the u half of a neighbour-record buffer or SoA arrays
-__global__ void k_gather_field(int64_t npad, int dim, Ax ax, const int32_t *__restrict__ perm, const double2 *__restrict__ nb,
+__global__ void k_gather_field(int64_t npad, int dim, Ax ax, const int32_t *__restrict__ perm, const double2 *__restrict__ nb, bool lattice,
                                const double *__restrict__ s0, const double *__restrict__ s1,
                                const double *__restrict__ s2, double *dst) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -40,7 +40,7 @@ __global__ void k_gather_field(int64_t npad, int dim, Ax ax, const int32_t *__re
   const double *s[3] = {s0, s1, s2};
   int32_t uidx = perm[i];
   if (uidx < 0) return;
-  for (int k = 0; k < dim; ++k) dst[(int64_t)dim * uidx + ax.a[k]] = nb ? nb[pd_elem(i) + 32 * k].y : s[k][i];
+  for (int k = 0; k < dim; ++k) dst[(int64_t)dim * uidx + ax.a[k]] = nb ? nb[pd_pair_index(lattice, npad, i, k)].y : s[k][i];
 }
 
 // scalar per node
@@ -93,7 +93,7 @@ int get_field(pd_sim *s, double *dst, bool velocity) {
   if (!s || !dst) { pdi::set_error("null argument"); return PD_ERR_ARG; }
   DevTmp tmp(s, sizeof(double) * s->dim * s->n);
   if (!tmp.p) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
-  k_gather_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, velocity ? nullptr : s->nb[s->cur],
+  k_gather_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, velocity ? nullptr : s->nb[s->cur], s->lat.on,
                                                        s->v[0], s->v[1], s->v[2], (double *)tmp.p);
   PD_CUDA(cudaGetLastError());
   return copy_out(s, dst, tmp.p, sizeof(double) * s->dim * s->n);
@@ -209,11 +209,11 @@ int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volum
   }
   if (!ok) { pdi::set_error("device allocation failed for the state arrays"); return fail(PD_ERR_ALLOC); }
   k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, (const double *)d_u0, s->flags, true,
-                                                         s->nb[0], nullptr, nullptr, nullptr);
+                                                         s->nb[0], s->lat.on, nullptr, nullptr, nullptr);
   k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, (const double *)d_v0, s->flags, true,
-                                                         nullptr, s->v[0], s->v[1], s->v[2]);
+                                                         nullptr, false, s->v[0], s->v[1], s->v[2]);
   k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, (const double *)d_val, s->flags, false,
-                                                         nullptr, s->bval[0], s->bval[1], s->bval[2]);
+                                                         nullptr, false, s->bval[0], s->bval[1], s->bval[2]);
   cudaError_t e = cudaGetLastError();
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
   if (e != cudaSuccess) return fail(pdi::cuda_fail(e, "pd_create state initialisation"));

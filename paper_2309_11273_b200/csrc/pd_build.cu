@@ -40,16 +40,7 @@ namespace {
 
 constexpr int TPB = 256;
 
-struct Grid {
-  double lo[3];
-  double inv_c[3];  // 1 / cell edge per dimension
-  int nc[3];        // cells per dim
-  int S[3];         // search radius in cells per dim
-  int dim;
-  int ax[3];        // internal axis k = user axis ax[k]
-  int R, BZ;        // rows per thread, z-levels per tile
-  int ncyg, nczt, maxchunk;
-};
+using Grid = PdGrid;
 
 __device__ __forceinline__ void cell_of(const Grid &g, const double *p, int *q) {
 #pragma unroll
@@ -754,6 +745,14 @@ int build_family(pd_sim *s, const double *coords, const double *vol, const uint8
   PD_CUDA(cudaMemsetAsync(row_end, 0, sizeof(int32_t) * nrow, st));
   k_tables<<<nblk(n), TPB, 0, st>>>(n, g.nc[0], keys2, cell_start, cell_end, row_start, row_end);
 
+  // ---- lattice body (one node per cell, uniform volume, small stencil)?  then the dense layout of
+  //      pd_lattice.cu replaces everything below ----
+  {
+    int rc = build_lattice(s, g, coords, vol, flags, precut, n_precut, keys2, ord1, cell_start, cell_end);
+    if (rc < 0) return rc;
+    if (rc == 1) return PD_OK;
+  }
+
   // ---- 3. lanes, tiles, final order ----
   SCRATCH(rowid, int32_t, n);
   SCRATCH(tval, int32_t, n);
@@ -911,7 +910,10 @@ int export_bond_mask(pd_sim *s, long long *rowptr_dev, int32_t *col_dev, uint8_t
     tmp = dev_alloc(s, tb ? tb : 1);
     if (!tmp) { set_error("device allocation failed"); rc = PD_ERR_ALLOC; break; }
     if (cub::DeviceScan::ExclusiveSum(tmp, tb, cnt, rowptr_dev, (int)(n + 1), st) != cudaSuccess) { rc = PD_ERR_CUDA; break; }
-    if (col_dev && intact_dev)
+    if (col_dev && intact_dev && s->lat.on) {
+      cudaStreamSynchronize(st);
+      rc = lat_export_bond_mask(s, rowptr_dev, col_dev, intact_dev);
+    } else if (col_dev && intact_dev)
       k_export_rows<<<nblk(s->ngroups * 32), TPB, 0, st>>>(s->ngroups, s->perm, rowptr_dev, s->goff, s->soff, s->col,
                                                             s->member, s->seg, col_dev, intact_dev);
     if (cudaGetLastError() != cudaSuccess) rc = PD_ERR_CUDA;

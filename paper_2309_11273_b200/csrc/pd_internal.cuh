@@ -55,6 +55,11 @@ __host__ __device__ __forceinline__ int64_t pd_elem_inv(uint32_t e) {
   return ((int64_t)(e / (32 * PD_NP)) << 5) | (e & 31);
 }
 
+// double2 index of pair p of node i in a neighbour-record buffer, for either layout
+__host__ __device__ __forceinline__ int64_t pd_pair_index(bool lattice, int64_t npad, int64_t i, int p) {
+  return lattice ? (int64_t)p * npad + i : (int64_t)pd_elem(i) + 32 * p;
+}
+
 // Calls f(s, bit, r, k) for every bond slot of one lane: s = segment index inside the group,
 // bit = 4 t + r, k = entry index inside the group.  `words` = the lane's segment words (any of
 // seg / member / nofail: only the CODE nibble is read here), stride 32.
@@ -78,7 +83,47 @@ __host__ __device__ __forceinline__ void pd_for_lane_slots(const uint32_t *words
   }
 }
 
+// ---- dense lattice layout (pd_lattice.cu), used when the body is a (jittered) lattice with one node
+// per cell, uniform volume and a family stencil of <= 128 relative offsets.  Nodes live in a dense
+// array over the cell grid (internal axes 0 = lane axis X, 1 = Y, 2 = Z) with a margin of the
+// stencil radius on every side (zero-filled PHANTOM cells):
+//     cell (x, y, z) -> final index  ((z + HZ) * DY + (y + HY)) * DX + (x + HX)
+//   neighbour-record pair p of node i sits at nb[b][p * npad + i]  (each pair a dense 3-D array)
+//   lmask / lmember / lnofail [w * npad + i], w < 4: one bit per stencil offset (bit order = the
+//   column table below), so no neighbour index is stored at all.
+// The stencil is a table of COLUMNS: offsets (dx, dy0 .. dy0 + n - 1, dz), n <= 7, whose bits
+// bit0 .. bit0 + n - 1 lie inside one mask word.
+#define PD_LAT_MAXCOL 160
+struct PdLatCol {
+  int16_t dx, dy0, dz;
+  uint8_t n, word, bit0, split, pad0, pad1;   // split: which warp of a row group walks this column
+};
+struct PdGrid {
+  double lo[3];
+  double inv_c[3];  // 1 / cell edge per dimension
+  int nc[3];        // cells per dim
+  int S[3];         // search radius in cells per dim
+  int dim;
+  int ax[3];        // internal axis k = user axis ax[k]
+  int R, BZ;        // rows per thread, z-levels per tile
+  int ncyg, nczt, maxchunk;
+};
+struct PdLattice {
+  bool on = false;
+  int DX = 0, DY = 0, DZ = 0;      // dense dims incl. margins
+  int HX = 0, HY = 0, HZ = 0;      // margins = stencil radius per axis
+  int PX = 0, PY = 0, PZ = 0;      // padded cell counts (PX multiple of 32, PY of 4)
+  int ncol = 0, nbits = 0, nw = 0; // columns, mask bits used (incl. padding), mask words
+  uint32_t fullw[4] = {0, 0, 0, 0};
+  PdLatCol cols[PD_LAT_MAXCOL];
+  uint32_t *mask = nullptr, *member = nullptr, *nofail = nullptr;   // [4][npad]
+  uint8_t *rgocc = nullptr;        // [PZ][PY/4][PX/32]: the 32x4 row group holds a node
+  int32_t *off2bit = nullptr;      // [(2S2+1)(2S1+1)(2S0+1)] offset -> bit index or -1
+  int S[3] = {0, 0, 0};
+};
+
 struct pd_sim {
+  PdLattice lat;
   // scalars
   int dim = 0, mode = 0;
   int ax[3] = {0, 1, 2};        // internal component k = user component ax[k]; internal 0 is the lane axis
@@ -124,6 +169,15 @@ void dev_free_all(pd_sim *s);
 int build_family(pd_sim *s, const double *coords_user_dev, const double *vol_user_dev,
                  const uint8_t *flags_user_dev, const int32_t *precut_dev, int64_t n_precut);
 int export_bond_mask(pd_sim *s, long long *rowptr_dev, int32_t *col_dev, uint8_t *intact_dev);
+// pd_lattice.cu: returns 1 if the lattice layout was built, 0 if the body does not qualify, < 0 on error
+int build_lattice(pd_sim *s, const PdGrid &g, const double *coords_user_dev, const double *vol_user_dev,
+                  const uint8_t *flags_user_dev, const int32_t *precut_dev, int64_t n_precut,
+                  const uint32_t *keys_sorted, const int32_t *ids_sorted, const int32_t *cell_start,
+                  const int32_t *cell_end);
+int lat_export_bond_mask(pd_sim *s, const long long *rowptr_dev, int32_t *col_dev, uint8_t *intact_dev);
+int lat_launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
+int lat_launch_force_update(pd_sim *s);
+int lat_launch_damage(pd_sim *s);
 // pd_step.cu
 int launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
 int launch_force_update(pd_sim *s);

@@ -373,6 +373,7 @@ void force_dispatch(const StepArgs &a, bool univ, unsigned grid, cudaStream_t st
 namespace pdi {
 
 int launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
+  if (s->lat.on) return lat_launch_dilatation(s, theta_out, do_break);
   StepArgs a = make_args(s);
   a.theta_out = theta_out;
   const bool frac = do_break && s->fracture;
@@ -382,6 +383,7 @@ int launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
 }
 
 int launch_force_update(pd_sim *s) {
+  if (s->lat.on) return lat_launch_force_update(s);
   StepArgs a = make_args(s);
   a.nbw = s->nb[s->cur ^ 1];
   if (s->dim == 2) force_dispatch<2>(a, s->uniform_v, ngrid(s), s->stream);
@@ -390,6 +392,7 @@ int launch_force_update(pd_sim *s) {
 }
 
 int launch_damage(pd_sim *s) {
+  if (s->lat.on) return lat_launch_damage(s);
   StepArgs a = make_args(s);
   cudaMemsetAsync(s->stats_dev, 0, 3 * sizeof(unsigned long long), s->stream);
   k_damage<<<ngrid(s), TPB, 0, s->stream>>>(a, s->uniform_v);
