@@ -180,7 +180,7 @@ int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volum
   void *d_coords = nullptr, *d_vol = nullptr, *d_flags = nullptr, *d_precut = nullptr, *d_u0 = nullptr, *d_v0 = nullptr,
        *d_val = nullptr;
   const int dim = s->dim;
-  auto fail = [&](int code) { pdi::dev_free_all(s); delete s; return code; };
+  auto fail = [&](int code) { pdi::lat_free_cache(s); pdi::dev_free_all(s); delete s; return code; };
   if ((rc = stage(s, coords, sizeof(double) * dim * n, &d_coords))) return fail(rc);
   if ((rc = stage(s, volumes, sizeof(double) * n, &d_vol))) return fail(rc);
   if (bc) {
@@ -334,6 +334,7 @@ int pd_get_layout(pd_sim *s, int64_t counts[8]) {
 
 int pd_destroy(pd_sim *s) {
   if (!s) return PD_OK;
+  pdi::lat_free_cache(s);
   pdi::dev_free_all(s);
   delete s;
   return PD_OK;

@@ -32,20 +32,35 @@ __device__ __forceinline__ double dot3(const double *x, const double *y) {
   return d;
 }
 
-// dilatation (+ break) policy: R rows per lane
-template <int DIM, bool FRAC, bool UNIV, int R>
+// dilatation (+ break) policy: R rows per lane.
+// FILT (lattice layout): the fast pass does not evaluate dot - s_c ||xi||^2 per bond; it keeps the
+// maximum of the HIGH WORDS of dot over a step and compares it with the high word of
+// thr = s_c * min ||xi||^2 of that stencil offset (a static lower bound over all bonds, pd_lattice.cu):
+// hi(dot) < hi(thr) => dot < thr <= s_c ||xi||^2 => the exact test is negative.  Anything else sends
+// the bonds to the masked variant, which evaluates the exact test.  (Integer compares on the ALU pipe
+// instead of 4 FP64 instructions per bond.)
+template <int DIM, bool FRAC, bool UNIV, int R, bool FILT = false>
 struct DilPolicy {
   using E = Ent<DIM, false, !UNIV>;
   static constexpr bool kFrac = FRAC;
   double xo[R][DIM], uo[R][DIM], acc[R], snap[R];
   double s_c;
   int sg;   // AND of the sign words of dot - s_c r2 over the fast path's bonds
+  int mxhi; // FILT: max high word of dot over the bonds of the current step
 
   __device__ __forceinline__ void fast_begin() {
     if (FRAC) {
 #pragma unroll
       for (int r = 0; r < R; ++r) snap[r] = acc[r];
       sg = (int)0x80000000;
+      mxhi = (int)0x80000000;
+    }
+  }
+  // FILT: end of a fast step whose bonds share the threshold high word thr_hi
+  __device__ __forceinline__ void step_end(int thr_hi) {
+    if (FRAC && FILT) {
+      if (mxhi >= thr_hi) sg = 0;
+      mxhi = (int)0x80000000;
     }
   }
   // true: some bond of the fast pass met the break criterion on some lane; the accumulators are
@@ -69,7 +84,9 @@ struct DilPolicy {
     const double dot = dot3<DIM>(xi, eta);
     bool brk = false;
     if (!MASKED) in = true;
-    if (FRAC) {
+    if (FRAC && FILT && !MASKED) {
+      mxhi = max(mxhi, __double2hiint(dot));
+    } else if (FRAC) {
       // s >= s_c breaks (Eq. 1.30): xi.eta - s_c ||xi||^2 >= 0, one rounding, sign read off the high word
       const double t = fma(-s_c, dot3<DIM>(xi, xi), dot);
       if (MASKED) {
@@ -101,6 +118,7 @@ struct ForcePolicy {
   double xo[R][DIM], uo[R][DIM], f[R][DIM], cth_i[R], gmu_i[R];
 
   __device__ __forceinline__ void fast_begin() {}
+  __device__ __forceinline__ void step_end(int) {}
   __device__ __forceinline__ bool fast_failed() { return false; }
   template <bool MASKED>
   __device__ __forceinline__ bool bond(int r, const E &e, bool in, bool) {

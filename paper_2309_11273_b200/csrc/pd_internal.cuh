@@ -117,8 +117,13 @@ struct PdLattice {
   uint32_t fullw[4] = {0, 0, 0, 0};
   PdLatCol cols[PD_LAT_MAXCOL];
   uint32_t *mask = nullptr, *member = nullptr, *nofail = nullptr;   // [4][npad]
-  uint8_t *rgocc = nullptr;        // [PZ][PY/4][PX/32]: the 32x4 row group holds a node
+  uint8_t *rgocc = nullptr;        // [PZ + 8][(PY + 8)/4][PX/32]: the 32x4 row group holds a node
+  uint32_t *flags32 = nullptr;     // [npad] the node flags as 32-bit words (4-byte asynchronous copies)
   int32_t *off2bit = nullptr;      // [(2S2+1)(2S1+1)(2S0+1)] offset -> bit index or -1
+  double r2lb[128];                // per stencil bit: min over all bonds of ||xi||^2 exactly as the step kernels
+                                   // compute it (break-test filter: dot < s_c * r2lb  =>  the bond cannot break)
+  void *cache[2] = {nullptr, nullptr};   // host: prepared launch arguments of the two step kernels (pd_lattice_step.cu)
+  int32_t *thr_dev = nullptr;      // device: per (column, step) filter thresholds of the dilatation kernel
   int S[3] = {0, 0, 0};
 };
 
@@ -178,6 +183,7 @@ int lat_export_bond_mask(pd_sim *s, const long long *rowptr_dev, int32_t *col_de
 int lat_launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
 int lat_launch_force_update(pd_sim *s);
 int lat_launch_damage(pd_sim *s);
+void lat_free_cache(pd_sim *s);
 // pd_step.cu
 int launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
 int launch_force_update(pd_sim *s);

@@ -8,13 +8,7 @@
 // 128-bit mask over the stencil (bond exists and is unbroken, Eq. 1.30).  Exactly the same families
 // as the general layout: membership is decided by the same exact distance test per node pair.
 //
-// Step kernels: one CTA per spatial TILE of 32 x TY x TZ cells.  The neighbour records of the tile
-// plus a halo of the stencil radius are staged in shared memory with 16-byte asynchronous copies
-// (cp.async) -- every HBM/L2 access of the step is a coalesced bulk row copy, the ~120 gathers per
-// node are shared-memory reads.  A warp owns a ROW GROUP (32 lanes x 4 rows adjacent in y); the
-// stencil columns (dx, dy0..dy0+n-1, dz) are walked with a 4-entry register window sliding along y
-// exactly as in pd_step.cu (one shared-memory record per 4 bonds), NSPLIT warps share a row group
-// by splitting the columns between them and add their partial sums through shared memory.
+// This file is the builder of that layout; the step kernels are in pd_lattice_step.cu.
 #include <cub/device/device_reduce.cuh>
 #include <cub/iterator/transform_input_iterator.cuh>
 
@@ -88,8 +82,8 @@ __global__ void k_lat_offsets(int64_t n, PdGrid g, double h2, const double *__re
 __global__ void k_lat_place(int64_t n, PdGrid g, LatDims L, const double *__restrict__ coords,
                             const double *__restrict__ vol, const uint8_t *__restrict__ flags,
                             const uint32_t *__restrict__ keys, const int32_t *__restrict__ ids, int32_t *perm,
-                            int32_t *iperm, double2 *nb0, double2 *nb1, double *volF, uint8_t *flagsF, uint8_t *rgocc,
-                            int nxc, int nyq) {
+                            int32_t *iperm, double2 *nb0, double2 *nb1, double *volF, uint8_t *flagsF, uint32_t *flags32,
+                            uint8_t *rgocc, int nxc, int nyq) {
   int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= n) return;
   const uint32_t key = keys[p];
@@ -110,6 +104,7 @@ __global__ void k_lat_place(int64_t n, PdGrid g, LatDims L, const double *__rest
     if (f & (8u << g.ax[k])) fi |= 8u << k;
   }
   flagsF[i] = (uint8_t)fi;
+  flags32[i] = fi;
   rgocc[((int64_t)cz * nyq + (cy >> 2)) * nxc + (cx >> 5)] = 1;
 }
 
@@ -117,7 +112,7 @@ __global__ void k_lat_place(int64_t n, PdGrid g, LatDims L, const double *__rest
 __global__ void k_lat_masks(LatDims L, int dim, int nbits, double h2, double G, const int4 *__restrict__ offs,
                             const int32_t *__restrict__ perm, double2 *nb0, double2 *nb1,
                             const double *__restrict__ vol, double *mF, double *minvF, double *fvolF, int32_t *rowlen,
-                            uint32_t *member) {
+                            uint32_t *member, unsigned long long *r2lb) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= L.npad || perm[i] < 0) return;
   double pi[3] = {0, 0, 0};
@@ -135,6 +130,14 @@ __global__ void k_lat_masks(LatDims L, int dim, int nbits, double h2, double G, 
     const double r2 = dist2_exact(dim, pi, pj);
     if (r2 <= h2) {
       w[b >> 5] |= 1u << (b & 31);
+      {   // lower bound of ||xi||^2 per stencil offset, in the step kernels' own arithmetic (pd_bond.cuh dot3)
+        double xi[3] = {0, 0, 0};
+        for (int k = 0; k < dim; ++k) xi[k] = pj[k] - pi[k];
+        double rk = __dmul_rn(xi[0], xi[0]);
+        for (int k = 1; k < dim; ++k) rk = fma(xi[k], xi[k], rk);
+        const unsigned long long bitsr = (unsigned long long)__double_as_longlong(rk);   // rk > 0: bit order = value order
+        if (bitsr < r2lb[b]) atomicMin(&r2lb[b], bitsr);
+      }
       const double vj = vol[j];
       m = fma(r2, vj, m);
       fv += vj;
@@ -363,6 +366,8 @@ int build_lattice(pd_sim *s, const PdGrid &g, const double *coords, const double
   LAT_ALLOC(l.mask, uint32_t, 4 * s->npad);
   LAT_ALLOC(l.rgocc, uint8_t, (size_t)(l.PZ + 8) * nyq * nxc);
   LAT_ALLOC(l.off2bit, int32_t, nbox);
+  LAT_ALLOC(l.flags32, uint32_t, s->npad);
+  PD_CUDA(cudaMemsetAsync(l.flags32, 0, sizeof(uint32_t) * s->npad, st));
   PD_CUDA(cudaMemsetAsync(s->perm, 0xff, sizeof(int32_t) * s->npad, st));
   for (double *p : {s->vol, s->m, s->minv, s->fvol}) PD_CUDA(cudaMemsetAsync(p, 0, sizeof(double) * s->npad, st));
   PD_CUDA(cudaMemsetAsync(s->flags, 0, s->npad, st));
@@ -371,13 +376,26 @@ int build_lattice(pd_sim *s, const PdGrid &g, const double *coords, const double
   PD_CUDA(cudaMemsetAsync(l.rgocc, 0, (size_t)(l.PZ + 8) * nyq * nxc, st));
   PD_CUDA(cudaMemcpyAsync(l.off2bit, off2bit.data(), sizeof(int32_t) * nbox, cudaMemcpyHostToDevice, st));
   k_lat_place<<<nblk(n), TPB, 0, st>>>(n, g, L, coords, vol, flags, keys, ids, s->perm, s->iperm, s->nb[0], s->nb[1],
-                                       s->vol, s->flags, l.rgocc, nxc, nyq);
+                                       s->vol, s->flags, l.flags32, l.rgocc, nxc, nyq);
   l.on = true;   // from here on the allocations belong to the lattice layout (freed by pd_destroy / fail path)
   int4 *offs = make_offs_dev(s);
   if (!offs) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
   scratch.push_back(offs);
+  unsigned long long *r2lb_d = (unsigned long long *)salloc(sizeof(unsigned long long) * 128);
+  if (!r2lb_d) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
+  PD_CUDA(cudaMemsetAsync(r2lb_d, 0xff, sizeof(unsigned long long) * 128, st));
   k_lat_masks<<<nblk(s->npad), TPB, 0, st>>>(L, dim, l.nbits, h2, s->G, offs, s->perm, s->nb[0], s->nb[1], s->vol, s->m,
-                                             s->minv, s->fvol, s->rowlen, l.member);
+                                             s->minv, s->fvol, s->rowlen, l.member, r2lb_d);
+  {
+    unsigned long long hb2[128];
+    PD_CUDA(cudaMemcpyAsync(hb2, r2lb_d, sizeof(hb2), cudaMemcpyDeviceToHost, st));
+    PD_CUDA(cudaStreamSynchronize(st));
+    for (int b = 0; b < 128; ++b) {
+      double v = 0.0;
+      if (hb2[b] != ~0ull) memcpy(&v, &hb2[b], 8);
+      l.r2lb[b] = v;   // 0: no bond with this offset -> the filter never passes it
+    }
+  }
   PD_CUDA(cudaMemcpyAsync(l.mask, l.member, sizeof(uint32_t) * 4 * s->npad, cudaMemcpyDeviceToDevice, st));
 
   // ---- Z, checks ----
@@ -438,480 +456,3 @@ int lat_export_bond_mask(pd_sim *s, const long long *rowptr_dev, int32_t *col_de
 
 }  // namespace pdi
 
-// ================================================================================================
-// step kernels
-namespace {
-
-struct LatCol8 { int off; uint8_t n, word, bit0, pad; };   // off: smem offset (double2 units) of entry 0 relative to row 0's own cell
-
-struct LatArgs {
-  int DX, DY, HX, HY, HZ;
-  int nxc, nyt, nyq;                 // tiles along x and y; row groups along y (rgocc stride)
-  int TY, TZ, SX, SY, SZ;            // tile and shared-memory tile dims
-  int nsplit, nw;
-  int cbeg[5];                       // split s walks cols[cbeg[s] .. cbeg[s+1])
-  int64_t npad;
-  uint32_t fullw[4];
-  const double2 *nbr;                // pair arrays [PD_NP][npad] holding u^n (and cth^n)
-  double2 *nbw;                      // dilatation: the same buffer (pair AUX written); force: the other buffer
-  uint32_t *mask;
-  const uint32_t *nofail;
-  const uint8_t *rgocc;
-  const double *minv;
-  double *v[3];
-  const double *bval[3];
-  double *theta_out;
-  const uint8_t *flags;
-  const int32_t *perm;
-  double A, c1, G, s_c, vol_uniform, rho, dt, ramp_time;
-  int64_t step;
-  LatCol8 cols[PD_LAT_MAXCOL];
-};
-
-__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async4(void *smem_dst, const void *gsrc) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-
-// predicated 16-byte shared-memory load: no branch, so the four bonds of a step stay in one basic block
-__device__ __forceinline__ void lds_if(double2 &v, const double2 *ptr, uint32_t pred) {
-  const unsigned a = (unsigned)__cvta_generic_to_shared(ptr);
-  asm("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %3, 0;\n\t@p ld.shared.v2.f64 {%0, %1}, [%2];\n\t}"
-      : "+d"(v.x), "+d"(v.y) : "r"(a), "r"(pred));
-}
-
-template <int NPAIR, class E>
-__device__ __forceinline__ void lds_ent(E &e, const double2 *tile, int tsz, int idx) {
-  constexpr int DIMP = sizeof(e.p) / sizeof(double2);
-#pragma unroll
-  for (int k = 0; k < DIMP; ++k) e.p[k] = tile[k * tsz + idx];
-  if (NPAIR > DIMP) e.g = tile[DIMP * tsz + idx];
-}
-template <int NPAIR, class E>
-__device__ __forceinline__ void lds_ent_if(E &e, const double2 *tile, int tsz, int idx, uint32_t pred) {
-  constexpr int DIMP = sizeof(e.p) / sizeof(double2);
-#pragma unroll
-  for (int k = 0; k < DIMP; ++k) lds_if(e.p[k], tile + k * tsz + idx, pred);
-  if (NPAIR > DIMP) lds_if(e.g, tile + DIMP * tsz + idx, pred);
-}
-
-// one stencil column: n steps, row r of step t pairs with the record at base + (t + r) * SX
-template <bool MASKED, int NPAIR, class P>
-__device__ __forceinline__ void lat_run_col(P &p, const double2 *tile, int tsz, int base, int SX, int n,
-                                            const uint32_t (&bits)[4], const uint32_t (&nfb)[4], uint32_t (&clr)[4]) {
-  typename P::E S[4];
-#pragma unroll
-  for (int q = 0; q < 4; ++q) lds_ent<NPAIR>(S[q], tile, tsz, base + q * SX);
-  uint32_t anyp = 0;
-  if (MASKED) anyp = __reduce_or_sync(FULL, bits[0] | (bits[1] << 7) | (bits[2] << 14) | (bits[3] << 21));
-  auto bond = [&](int r, const typename P::E &e, int t) {
-    if (p.template bond<MASKED>(r, e, (bits[r] >> t) & 1u, (nfb[r] >> t) & 1u)) clr[r] |= 1u << t;
-  };
-#pragma unroll
-  for (int t = 0; t < PD_MAXSTEP; ++t) {
-    if (t < n) {
-      const bool live = !MASKED || (anyp & (0x204081u << t)) != 0;   // warp-uniform
-      if (live) bond(0, S[t % 4], t);
-      lds_ent_if<NPAIR>(S[t % 4], tile, tsz, base + (t + 4) * SX, (t + 1 < n) ? 1u : 0u);   // record t+4: row 3 of step t+1
-      if (live) {
-        bond(1, S[(t + 1) % 4], t);
-        bond(2, S[(t + 2) % 4], t);
-        bond(3, S[(t + 3) % 4], t);
-      }
-    }
-  }
-}
-
-// stages the tile, walks the columns of this warp's split, returns false if the warp has nothing to finish
-// (NPAIR pairs per record: DIM position pairs + the aux pair for the force pass)
-template <int DIM, int NPAIR, int MAXT, class P>
-__device__ __forceinline__ bool lat_tile(P &p, const LatArgs &a, double2 *sm, int64_t (&inode)[4], int &rg, int &sp,
-                                         uint32_t *&smask, int *&sflag, int &NT) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
-  const int xc = blockIdx.x, yt = blockIdx.y, zt = blockIdx.z;
-  const int x0 = xc * 32, y0 = yt * a.TY, z0 = zt * a.TZ;
-  const int nrgy = a.TY >> 2, nrg = nrgy * a.TZ;
-  NT = 32 * a.TY * a.TZ;
-  const int tsz = a.SZ * a.SY * a.SX;
-  smask = (uint32_t *)(sm + NPAIR * tsz + 4 * a.SX);
-  sflag = (int *)(smask + 4 * NT);
-  // ---- empty tile? ----
-  int occ = 0;
-  if ((int)threadIdx.x < nrg) {
-    const int rgy = threadIdx.x % nrgy, rgz = threadIdx.x / nrgy;
-    occ = a.rgocc[((int64_t)(z0 + rgz) * a.nyq + ((y0 >> 2) + rgy)) * a.nxc + xc];
-  }
-  if (!__syncthreads_or(occ)) return false;
-  // ---- stage the tile + halo: rows of SX records, 16-byte asynchronous copies ----
-  // (loops arranged so that no integer division by a run-time value is needed per row)
-  const int tyshift = a.TY == 8 ? 3 : 2;
-  for (int pl = warp; pl < NPAIR * a.SZ; pl += nwarp) {   // plane = (pair, z level)
-    int pp = 0, zz = pl;
-    while (zz >= a.SZ) { zz -= a.SZ; ++pp; }
-    const int gp = pp < DIM ? pp : PD_P_AUX;
-    const double2 *src = a.nbr + (int64_t)gp * a.npad + ((int64_t)(z0 + zz) * a.DY + y0) * a.DX + x0 + lane;
-    double2 *dst = sm + (int64_t)pl * a.SY * a.SX + lane;
-    const bool two = lane + 32 < a.SX;
-    for (int yy = 0; yy < a.SY; ++yy) {
-      cp_async16(dst, src);
-      if (two) cp_async16(dst + 32, src + 32);
-      src += a.DX;
-      dst += a.SX;
-    }
-  }
-  for (int w = 0; w < a.nw; ++w)
-    for (int tn = threadIdx.x; tn < NT; tn += blockDim.x) {
-      const int x = tn & 31, row = tn >> 5, y = row & (a.TY - 1), z = row >> tyshift;
-      const int64_t i = ((int64_t)(z0 + z + a.HZ) * a.DY + (y0 + y + a.HY)) * a.DX + (x0 + x + a.HX);
-      cp_async4(smask + w * NT + tn, a.mask + (int64_t)w * a.npad + i);
-    }
-  if (threadIdx.x == 0) *sflag = 0;
-  cp_async_wait_all();
-  __syncthreads();
-  // ---- this warp's row group and column split ----
-  rg = warp / a.nsplit;
-  sp = warp % a.nsplit;
-  const int rgy = rg % nrgy, rgz = rg / nrgy;
-  const bool active = a.rgocc[((int64_t)(z0 + rgz) * a.nyq + ((y0 >> 2) + rgy)) * a.nxc + xc] != 0;
-  int own0 = ((rgz + a.HZ) * a.SY + (rgy * 4 + a.HY)) * a.SX + lane + a.HX;
-  int tn0 = ((rgz * a.TY) + rgy * 4) * 32 + lane;
-#pragma unroll
-  for (int r = 0; r < 4; ++r)
-    inode[r] = ((int64_t)(z0 + rgz + a.HZ) * a.DY + (y0 + rgy * 4 + r + a.HY)) * a.DX + (x0 + lane + a.HX);
-  if (!active) return true;   // (still takes part in the reduction barriers; its sums are zero)
-#pragma unroll
-  for (int r = 0; r < 4; ++r) {
-#pragma unroll
-    for (int k = 0; k < DIM; ++k) {
-      const double2 xu = sm[k * tsz + own0 + r * a.SX];
-      p.xo[r][k] = xu.x;
-      p.uo[r][k] = xu.y;
-    }
-  }
-  for (int c = a.cbeg[sp]; c < a.cbeg[sp + 1]; ++c) {
-    const LatCol8 col = a.cols[c];
-    const int n = col.n;
-    const uint32_t nmask = (1u << n) - 1u;
-    uint32_t bits[4], nfb[4] = {0, 0, 0, 0}, clr[4] = {0, 0, 0, 0};
-#pragma unroll
-    for (int r = 0; r < 4; ++r) bits[r] = (smask[col.word * NT + tn0 + r * 32] >> col.bit0) & nmask;
-    const bool full = __all_sync(FULL, (bits[0] & bits[1] & bits[2] & bits[3]) == nmask);
-    bool slow = !full;
-    const int base = own0 + col.off;
-    if (!slow) {
-      p.fast_begin();
-      lat_run_col<false, NPAIR>(p, sm, tsz, base, a.SX, n, bits, nfb, clr);
-      slow = p.fast_failed();
-    }
-    if (slow) {
-      if (P::kFrac && a.nofail) {
-#pragma unroll
-        for (int r = 0; r < 4; ++r) nfb[r] = (a.nofail[(int64_t)col.word * a.npad + inode[r]] >> col.bit0) & nmask;
-      }
-      lat_run_col<true, NPAIR>(p, sm, tsz, base, a.SX, n, bits, nfb, clr);
-      if (P::kFrac) {
-        uint32_t anyclr = 0;
-#pragma unroll
-        for (int r = 0; r < 4; ++r) {
-          if (clr[r]) atomicAnd(&smask[col.word * NT + tn0 + r * 32], ~(clr[r] << col.bit0));
-          anyclr |= clr[r];
-        }
-        if (anyclr) *sflag = 1;
-      }
-    }
-  }
-  return true;
-}
-
-// partial sums of the NSPLIT warps of a row group are added through shared memory (the tile is dead by then)
-template <int NACC>
-__device__ __forceinline__ void lat_reduce(const LatArgs &a, double *red, int rg, int sp, double (&acc)[NACC]) {
-  const int lane = threadIdx.x & 31;
-  __syncthreads();   // every warp is done reading the tile
-  if (a.nsplit > 1) {
-    if (sp > 0) {
-#pragma unroll
-      for (int q = 0; q < NACC; ++q) red[((rg * (a.nsplit - 1) + sp - 1) * NACC + q) * 32 + lane] = acc[q];
-    }
-    __syncthreads();
-    if (sp == 0) {
-      for (int s2 = 1; s2 < a.nsplit; ++s2)
-#pragma unroll
-        for (int q = 0; q < NACC; ++q) acc[q] += red[((rg * (a.nsplit - 1) + s2 - 1) * NACC + q) * 32 + lane];
-    }
-  }
-}
-
-// broken bits back to HBM (only if some bond of the tile broke in this pass)
-__device__ __forceinline__ void lat_flush_masks(const LatArgs &a, const uint32_t *smask, const int *sflag, int NT) {
-  if (!*sflag) return;
-  const int xc = blockIdx.x, yt = blockIdx.y, zt = blockIdx.z;
-  const int x0 = xc * 32, y0 = yt * a.TY, z0 = zt * a.TZ;
-  const int tyshift = a.TY == 8 ? 3 : 2;
-  for (int w = 0; w < a.nw; ++w)
-    for (int tn = threadIdx.x; tn < NT; tn += blockDim.x) {
-      const int x = tn & 31, row = tn >> 5, y = row & (a.TY - 1), z = row >> tyshift;
-      const int64_t i = ((int64_t)(z0 + z + a.HZ) * a.DY + (y0 + y + a.HY)) * a.DX + (x0 + x + a.HX);
-      a.mask[(int64_t)w * a.npad + i] = smask[w * NT + tn];
-    }
-}
-
-template <int DIM, bool FRAC, int MAXT>
-__global__ void __launch_bounds__(MAXT) k_lat_dilatation(const __grid_constant__ LatArgs a) {
-  extern __shared__ __align__(16) double2 sm[];
-  const int lane = threadIdx.x & 31;
-  pdb::DilPolicy<DIM, FRAC, true, 4> p;
-  p.s_c = a.s_c;
-#pragma unroll
-  for (int r = 0; r < 4; ++r) p.acc[r] = 0.0;
-  int64_t inode[4];
-  int rg, sp, NT;
-  uint32_t *smask;
-  int *sflag;
-  if (!lat_tile<DIM, DIM, MAXT>(p, a, sm, inode, rg, sp, smask, sflag, NT)) return;
-  // the mask words must leave shared memory before the reduction reuses it
-  __syncthreads();
-  if (FRAC) lat_flush_masks(a, smask, sflag, NT);
-  lat_reduce<4>(a, (double *)sm, rg, sp, p.acc);
-  if (sp != 0) return;
-#pragma unroll
-  for (int r = 0; r < 4; ++r) {
-    const int64_t i = inode[r];
-    const double mi = a.minv[i];   // 0 for phantoms
-    const double theta = a.A * mi * (p.acc[r] * a.vol_uniform);
-    a.nbw[(int64_t)PD_P_AUX * a.npad + i] = make_double2(a.G * mi, a.c1 * theta * mi);
-    if (a.theta_out) a.theta_out[i] = theta;
-  }
-  (void)lane;
-}
-
-template <int DIM, int MAXT>
-__global__ void __launch_bounds__(MAXT) k_lat_force_update(const __grid_constant__ LatArgs a) {
-  extern __shared__ __align__(16) double2 sm[];
-  pdb::ForcePolicy<DIM, true, 4> p;
-#pragma unroll
-  for (int r = 0; r < 4; ++r) {
-    p.gmu_i[r] = p.cth_i[r] = 0.0;
-#pragma unroll
-    for (int k = 0; k < DIM; ++k) { p.f[r][k] = 0.0; p.xo[r][k] = p.uo[r][k] = 0.0; }
-  }
-  int64_t inode[4];
-  int rg, sp, NT;
-  uint32_t *smask;
-  int *sflag;
-  // own aux pair {G/m_i, cth_i}: read from HBM before the tile walk (coalesced; the copy in the tile is the same data)
-  {
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int xc = blockIdx.x, yt = blockIdx.y, zt = blockIdx.z;
-    const int nrgy = a.TY >> 2;
-    const int rg0 = warp / a.nsplit, rgy = rg0 % nrgy, rgz = rg0 / nrgy;
-#pragma unroll
-    for (int r = 0; r < 4; ++r) {
-      const int64_t i = ((int64_t)(zt * a.TZ + rgz + a.HZ) * a.DY + (yt * a.TY + rgy * 4 + r + a.HY)) * a.DX + (xc * 32 + lane + a.HX);
-      const double2 g = a.nbr[(int64_t)PD_P_AUX * a.npad + i];
-      p.gmu_i[r] = g.x;
-      p.cth_i[r] = g.y;
-    }
-  }
-  if (!lat_tile<DIM, DIM + 1, MAXT>(p, a, sm, inode, rg, sp, smask, sflag, NT)) return;
-  double acc[4 * DIM];
-#pragma unroll
-  for (int r = 0; r < 4; ++r)
-#pragma unroll
-    for (int k = 0; k < DIM; ++k) acc[r * DIM + k] = p.f[r][k];
-  lat_reduce<4 * DIM>(a, (double *)sm, rg, sp, acc);
-  if (sp != 0) return;
-  // ---- Eq. 2.11 + boundary dofs (App. B) ----
-  double g = 1.0;
-  if (a.ramp_time > 0.0) g = fmin(1.0, __ddiv_rn(__dmul_rn((double)a.step, a.dt), a.ramp_time));
-#pragma unroll
-  for (int r = 0; r < 4; ++r) {
-    const int64_t i = inode[r];
-    if (a.perm[i] < 0) continue;   // phantom
-    const unsigned fl = a.flags[i];
-#pragma unroll
-    for (int k = 0; k < DIM; ++k) {
-      const double fk = acc[r * DIM + k] * a.vol_uniform;
-      double vk = a.v[k][i];
-      double uk = p.uo[r][k];
-      if (fl & (1u << k)) {                       // clamped: u stays, v = 0
-        vk = 0.0;
-      } else if (fl & (8u << k)) {                // prescribed velocity
-        vk = a.bval[k][i];
-        uk = __dadd_rn(uk, __dmul_rn(a.dt, vk));
-      } else {
-        const double bk = (fl & PD_BODY_FORCE) ? a.bval[k][i] : 0.0;
-        const double ac = __ddiv_rn(__dadd_rn(fk, __dmul_rn(g, bk)), a.rho);
-        vk = __dadd_rn(vk, __dmul_rn(a.dt, ac));
-        uk = __dadd_rn(uk, __dmul_rn(a.dt, vk));
-      }
-      a.v[k][i] = vk;
-      a.nbw[(int64_t)k * a.npad + i] = make_double2(p.xo[r][k], uk);
-    }
-  }
-}
-
-}  // namespace
-
-namespace {
-
-// phi_i = 1 - sum_j rho_ij V_j / sum_j V_j (Eq. 1.31) and the three damage scalars
-__global__ void k_lat_damage(int64_t npad, int nw, double vol_uniform, const int32_t *__restrict__ perm,
-                             const uint32_t *__restrict__ mask, const int32_t *__restrict__ rowlen,
-                             const double *__restrict__ fvol, double *phi_out, unsigned long long *stats) {
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  unsigned long long broken = 0, ge_half = 0;
-  double phimax = 0.0;
-  if (i < npad && perm[i] >= 0) {
-    int cnt = 0;
-    for (int w = 0; w < nw; ++w) cnt += __popc(mask[(int64_t)w * npad + i]);
-    double sum = 0.0;   // the sum of cnt equal volumes, added one by one like sum_j V_j was
-    for (int q = 0; q < cnt; ++q) sum += vol_uniform;
-    const double phi = 1.0 - sum / fvol[i];
-    phi_out[i] = phi;
-    broken = (unsigned long long)(rowlen[i] - cnt);
-    ge_half = phi >= 0.5 ? 1ull : 0ull;
-    phimax = phi;
-  }
-  unsigned long long pbits = (unsigned long long)__double_as_longlong(fmax(phimax, 0.0));  // phi >= 0: bit order = value order
-  for (int o = 16; o > 0; o >>= 1) {
-    broken += __shfl_xor_sync(FULL, broken, o);
-    ge_half += __shfl_xor_sync(FULL, ge_half, o);
-    unsigned long long other = __shfl_xor_sync(FULL, pbits, o);
-    pbits = other > pbits ? other : pbits;
-  }
-  if ((threadIdx.x & 31) == 0) {
-    if (broken) atomicAdd(&stats[0], broken);
-    if (pbits) atomicMax(&stats[1], pbits);
-    if (ge_half) atomicAdd(&stats[2], ge_half);
-  }
-}
-
-int env_int(const char *name, int dflt) {
-  const char *e = getenv(name);
-  return e ? atoi(e) : dflt;
-}
-
-// tile shape, column table (shared-memory offsets, split between the warps of a row group) and pointers
-// npair = records pairs staged per node.  Returns the dynamic shared-memory size, 0 if nothing fits.
-size_t lat_make_args(pd_sim *s, LatArgs &a, int npair, int TY, int TZ, int nsplit) {
-  const PdLattice &l = s->lat;
-  a.DX = l.DX; a.DY = l.DY; a.HX = l.HX; a.HY = l.HY; a.HZ = l.HZ;
-  a.TY = TY; a.TZ = TZ;
-  a.SX = 32 + 2 * l.HX; a.SY = TY + 2 * l.HY; a.SZ = TZ + 2 * l.HZ;
-  a.nxc = l.PX / 32; a.nyt = (l.PY + TY - 1) / TY; a.nyq = (l.PY + 8) / 4;
-  a.nsplit = nsplit; a.nw = l.nw;
-  a.npad = s->npad;
-  for (int q = 0; q < 4; ++q) a.fullw[q] = l.fullw[q];
-  // greedy balance of the columns over the splits (by steps), longest first
-  std::vector<int> order(l.ncol), owner(l.ncol), load(nsplit, 0);
-  for (int c = 0; c < l.ncol; ++c) order[c] = c;
-  std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return l.cols[x].n > l.cols[y].n; });
-  for (int c : order) {
-    int best = 0;
-    for (int q = 1; q < nsplit; ++q) if (load[q] < load[best]) best = q;
-    owner[c] = best;
-    load[best] += l.cols[c].n + 1;
-  }
-  int k = 0;
-  for (int q = 0; q < nsplit; ++q) {
-    a.cbeg[q] = k;
-    for (int c = 0; c < l.ncol; ++c)
-      if (owner[c] == q) {
-        const PdLatCol &src = l.cols[c];
-        a.cols[k].off = (src.dz * a.SY + src.dy0) * a.SX + src.dx;
-        a.cols[k].n = src.n; a.cols[k].word = src.word; a.cols[k].bit0 = src.bit0; a.cols[k].pad = 0;
-        ++k;
-      }
-  }
-  for (int q = nsplit; q < 5; ++q) a.cbeg[q] = k;
-  a.nbr = s->nb[s->cur]; a.nbw = s->nb[s->cur];
-  a.mask = l.mask; a.nofail = l.nofail; a.rgocc = l.rgocc; a.minv = s->minv;
-  for (int q = 0; q < 3; ++q) { a.v[q] = s->v[q]; a.bval[q] = s->bval[q]; }
-  a.theta_out = nullptr; a.flags = s->flags; a.perm = s->perm;
-  a.A = s->A; a.c1 = s->c1; a.G = s->G; a.s_c = s->s_c; a.vol_uniform = s->vol_uniform; a.rho = s->rho; a.dt = s->dt;
-  a.ramp_time = s->ramp_time; a.step = s->step;
-  const size_t tile = (size_t)npair * a.SZ * a.SY * a.SX * sizeof(double2);
-  return tile + 4 * a.SX * sizeof(double2) + 4 * (size_t)(32 * TY * TZ) * sizeof(uint32_t) + 64;
-}
-
-constexpr size_t SMEM_MAX = 232448;   // 227 KB opt-in per CTA on sm_100
-
-// largest tile that fits: TZ from the preferred value down; TY = 4 (one row group along y) unless 2-D
-bool lat_pick(pd_sim *s, LatArgs &a, int npair, const char *env_prefix, int &TY, int &TZ, int &nsplit, size_t &smem) {
-  const int dim = s->dim;
-  char nm[64];
-  snprintf(nm, sizeof nm, "%s_TY", env_prefix); TY = env_int(nm, dim == 3 ? 4 : 8);
-  snprintf(nm, sizeof nm, "%s_TZ", env_prefix); TZ = env_int(nm, dim == 3 ? 4 : 1);
-  snprintf(nm, sizeof nm, "%s_NSPLIT", env_prefix); nsplit = env_int(nm, 0);
-  if (TY != 4 && TY != 8) TY = 4;
-  if (dim == 2) TZ = 1;
-  TZ = std::max(1, std::min(TZ, 8));
-  for (;; --TZ) {
-    smem = lat_make_args(s, a, npair, TY, TZ, 1);
-    if (smem <= SMEM_MAX) break;
-    if (TZ == 1) { if (TY == 8) { TY = 4; TZ = 2; continue; } return false; }
-  }
-  const int nrg = (TY / 4) * TZ;
-  if (nsplit <= 0) nsplit = std::max(1, std::min(4, 12 / nrg));   // about 8-12 warps per CTA
-  nsplit = std::max(1, std::min(nsplit, 4));
-  smem = lat_make_args(s, a, npair, TY, TZ, nsplit);
-  return true;
-}
-
-template <typename K>
-int lat_launch(K kernel, pd_sim *s, const LatArgs &a, int TY, int TZ, int nsplit, size_t smem) {
-  const PdLattice &l = s->lat;
-  const int nzt = (l.PZ + TZ - 1) / TZ;
-  const dim3 grid((unsigned)a.nxc, (unsigned)a.nyt, (unsigned)nzt);
-  const unsigned threads = (unsigned)((TY / 4) * TZ * nsplit * 32);
-  PD_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  kernel<<<grid, threads, smem, s->stream>>>(a);
-  return PD_OK;
-}
-
-}  // namespace
-
-namespace pdi {
-
-int lat_launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
-  LatArgs a;
-  int TY, TZ, nsplit;
-  size_t smem;
-  if (!lat_pick(s, a, s->dim, "PD_LAT_DIL", TY, TZ, nsplit, smem)) { set_error("lattice tile does not fit shared memory"); return PD_ERR_LIMIT; }
-  a.theta_out = theta_out;
-  const bool frac = do_break && s->fracture;
-  constexpr int MT = 384;
-  if ((TY / 4) * TZ * nsplit * 32 > MT) { set_error("lattice dilatation: too many threads per tile"); return PD_ERR_LIMIT; }
-  if (s->dim == 2) return frac ? lat_launch(k_lat_dilatation<2, true, MT>, s, a, TY, TZ, nsplit, smem)
-                               : lat_launch(k_lat_dilatation<2, false, MT>, s, a, TY, TZ, nsplit, smem);
-  return frac ? lat_launch(k_lat_dilatation<3, true, MT>, s, a, TY, TZ, nsplit, smem)
-              : lat_launch(k_lat_dilatation<3, false, MT>, s, a, TY, TZ, nsplit, smem);
-}
-
-int lat_launch_force_update(pd_sim *s) {
-  LatArgs a;
-  int TY, TZ, nsplit;
-  size_t smem;
-  if (!lat_pick(s, a, s->dim + 1, "PD_LAT_FRC", TY, TZ, nsplit, smem)) { set_error("lattice tile does not fit shared memory"); return PD_ERR_LIMIT; }
-  a.nbw = s->nb[s->cur ^ 1];
-  constexpr int MT = 384;
-  while ((TY / 4) * TZ * nsplit * 32 > MT && nsplit > 1) { --nsplit; smem = lat_make_args(s, a, s->dim + 1, TY, TZ, nsplit); a.nbw = s->nb[s->cur ^ 1]; }
-  if ((TY / 4) * TZ * nsplit * 32 > MT) { set_error("lattice force: too many threads per tile"); return PD_ERR_LIMIT; }
-  if (s->dim == 2) return lat_launch(k_lat_force_update<2, MT>, s, a, TY, TZ, nsplit, smem);
-  return lat_launch(k_lat_force_update<3, MT>, s, a, TY, TZ, nsplit, smem);
-}
-
-int lat_launch_damage(pd_sim *s) {
-  cudaMemsetAsync(s->stats_dev, 0, 3 * sizeof(unsigned long long), s->stream);
-  k_lat_damage<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->lat.nw, s->vol_uniform, s->perm, s->lat.mask, s->rowlen,
-                                                     s->fvol, s->phi, s->stats_dev);
-  return PD_OK;
-}
-
-}  // namespace pdi

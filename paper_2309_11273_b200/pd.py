@@ -13,7 +13,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIBPATH = os.path.join(_HERE, "libpd.so")
+_LIBPATH = os.environ.get("PD_LIBPATH") or os.path.join(_HERE, "libpd.so")   # PD_LIBPATH: an alternative build (debugging)
 
 PD_OK, PD_ERR_ARG, PD_ERR_ISOLATED, PD_ERR_ALLOC, PD_ERR_CUDA, PD_ERR_LIMIT = 0, -1, -2, -3, -4, -5
 EXPORTS = ["pd_create", "pd_step", "pd_get_u", "pd_get_v", "pd_get_damage", "pd_destroy", "pd_get_stats",
