@@ -122,8 +122,8 @@ struct PdLattice {
   int32_t *off2bit = nullptr;      // [(2S2+1)(2S1+1)(2S0+1)] offset -> bit index or -1
   double r2lb[128];                // per stencil bit: min over all bonds of ||xi||^2 exactly as the step kernels
                                    // compute it (break-test filter: dot < s_c * r2lb  =>  the bond cannot break)
-  void *cache[2] = {nullptr, nullptr};   // host: prepared launch arguments of the two step kernels (pd_lattice_step.cu)
-  int32_t *thr_dev = nullptr;      // device: per (column, step) filter thresholds of the dilatation kernel
+  void *cache[4] = {nullptr, nullptr, nullptr, nullptr};   // host: prepared launch arguments of the step kernels (pd_lattice_step.cu)
+  int32_t *thr_dev = nullptr, *thr_dir = nullptr;   // device: per (column, step) filter thresholds of the dilatation kernels
   int S[3] = {0, 0, 0};
 };
 

@@ -100,7 +100,7 @@ __device__ __forceinline__ void lds_ent_if(E &e, const double2 *plane, int psz, 
 template <bool MASKED, int NPAIR, class P>
 __device__ __forceinline__ void lat_run_col(P &p, const double2 *plane, int psz, int base, int SX, int n,
                                             const uint32_t (&bits)[4], const uint32_t (&nfb)[4], uint32_t (&clr)[4],
-                                            const int (&thr)[8]) {
+                                            const int *thr) {
   typename P::E S[4];
 #pragma unroll
   for (int q = 0; q < 4; ++q) lds_ent<NPAIR>(S[q], plane, psz, base + q * SX);
@@ -120,7 +120,7 @@ __device__ __forceinline__ void lat_run_col(P &p, const double2 *plane, int psz,
         bond(2, S[(t + 2) % 4], t);
         bond(3, S[(t + 3) % 4], t);
       }
-      if (!MASKED) p.step_end(thr[t]);
+      if (!MASKED && P::kFrac) p.step_end(thr[t]);
     }
   }
 }
@@ -134,9 +134,10 @@ template <int DIM, bool FRAC> struct PolicyOf<DIM, true, FRAC> { using type = pd
 
 // shared-memory carve-up (bytes), the same on host and device
 struct LatSmem {
-  size_t ring, smask, sepi, sfl, red, sdirty, total;
+  size_t ring, smask, sepi, sfl, red, scol, sthr, sdirty, total;
 };
-__host__ __device__ inline LatSmem lat_smem(int npair, int epi, bool force, int NP, int SY, int SX, int TY, int nsplit, int nacc) {
+__host__ __device__ inline LatSmem lat_smem(int npair, int epi, bool force, int NP, int SY, int SX, int TY, int nsplit, int nacc,
+                                            int ncol) {
   LatSmem m;
   const size_t NTL = 32 * (size_t)TY;
   m.ring = 0;
@@ -144,7 +145,9 @@ __host__ __device__ inline LatSmem lat_smem(int npair, int epi, bool force, int 
   m.sepi = m.smask + 2 * 4 * NTL * sizeof(uint32_t);
   m.sfl = m.sepi + 2 * (size_t)epi * NTL * sizeof(double);
   m.red = m.sfl + (force ? 2 * NTL * sizeof(uint32_t) : 0);
-  m.sdirty = m.red + (size_t)(TY / 4) * nsplit * nacc * 32 * sizeof(double);
+  m.scol = m.red + (size_t)(TY / 4) * nsplit * nacc * 32 * sizeof(double);
+  m.sthr = m.scol + (size_t)ncol * sizeof(LatCol8);                  // column table
+  m.sdirty = m.sthr + (force ? 0 : (size_t)ncol * 8 * sizeof(int));  // filter thresholds (dilatation)
   m.total = m.sdirty + 16;
   return m;
 }
@@ -160,19 +163,27 @@ __global__ void __launch_bounds__(MAXT) k_lat_march(const __grid_constant__ LatA
   const int xc = blockIdx.x, x0 = xc * 32, y0 = blockIdx.y * a.TY, z_lo = blockIdx.z * a.LZ, z_hi = min(z_lo + a.LZ, a.PZ);
   const int nrg = a.TY >> 2, NTL = 32 * a.TY;
   const int psz = a.SY * a.SX, plsz = NPAIR * psz;
-  const LatSmem lay = lat_smem(NPAIR, EPI, FORCE, a.NP, a.SY, a.SX, a.TY, a.nsplit, NACC);
+  const LatSmem lay = lat_smem(NPAIR, EPI, FORCE, a.NP, a.SY, a.SX, a.TY, a.nsplit, NACC, a.cbeg[MAXSPLIT]);
   double2 *ring = (double2 *)(smraw + lay.ring);
   uint32_t *smask = (uint32_t *)(smraw + lay.smask);   // [2][4][NTL]
   double *sepi = (double *)(smraw + lay.sepi);         // [2][EPI][NTL]: minv (dilatation) / v (force)
   uint32_t *sfl = (uint32_t *)(smraw + lay.sfl);       // [2][NTL] flags (force)
   double *red = (double *)(smraw + lay.red);           // [nrg][nsplit][NACC][32]
   int *sdirty = (int *)(smraw + lay.sdirty);           // [2]
+  LatCol8 *scol = (LatCol8 *)(smraw + lay.scol);       // the column table (shared-memory copy: short, fixed latency)
+  int *sthr = (int *)(smraw + lay.sthr);               // [ncol][8] break-filter thresholds
 
   // ---- nothing to do in this column segment? ----
   int occ = 0;
   for (int z = z_lo + tid; z < z_hi; z += nthr)
     for (int q = 0; q < nrg; ++q) occ |= a.rgocc[((int64_t)z * a.nyq + ((y0 >> 2) + q)) * a.nxc + xc];
   if (!__syncthreads_or(occ)) return;
+  {
+    const int ncol = a.cbeg[MAXSPLIT];
+    for (int c = tid; c < ncol; c += nthr) scol[c] = a.cols[c];
+    if (!FORCE && a.thr)
+      for (int c = tid; c < ncol * 8; c += nthr) sthr[c] = a.thr[c];
+  }
 
   auto load_plane = [&](int pz, int slot) {   // cell level pz (may be in the margin) -> ring slot
     for (int pp = 0; pp < NPAIR; ++pp) {
@@ -217,6 +228,10 @@ __global__ void __launch_bounds__(MAXT) k_lat_march(const __grid_constant__ LatA
 #else
 #define STAMP(k)
 #endif
+  // which levels hold a node of this warp's row group (read once: no global load inside the level loop)
+  unsigned long long actbits = 0;
+  for (int z = z_lo; z < z_hi; ++z)
+    if (a.rgocc[((int64_t)z * a.nyq + ((y0 >> 2) + rg)) * a.nxc + xc]) actbits |= 1ull << (z - z_lo);
   // which sums this warp finishes after the level's barrier: q = sp, sp + nsplit, ...
   uint32_t mine = 0;
   for (int q = sp; q < NACC; q += a.nsplit) mine |= 1u << q;
@@ -233,7 +248,7 @@ __global__ void __launch_bounds__(MAXT) k_lat_march(const __grid_constant__ LatA
       cp_async_commit();
     }
     STAMP(2)
-    const bool active = a.rgocc[((int64_t)z * a.nyq + ((y0 >> 2) + rg)) * a.nxc + xc] != 0;
+    const bool active = (actbits >> (z - z_lo)) & 1ull;
     P p;
     double acc[NACC];
     if (active) {
@@ -265,7 +280,7 @@ __global__ void __launch_bounds__(MAXT) k_lat_march(const __grid_constant__ LatA
       }
       const uint32_t *mk = smask + buf * 4 * NTL + tn0;
       for (int c = a.cbeg[sp]; c < a.cbeg[sp + 1]; ++c) {
-        const LatCol8 col = a.cols[c];
+        const LatCol8 col = scol[c];
         const int n = col.n;
         const uint32_t nmask = (1u << n) - 1u;
         uint32_t bits[4], nfb[4] = {0, 0, 0, 0}, clr[4] = {0, 0, 0, 0};
@@ -276,11 +291,7 @@ __global__ void __launch_bounds__(MAXT) k_lat_march(const __grid_constant__ LatA
         if (s2 >= a.NP) s2 -= a.NP;
         const double2 *pl = ring + (int64_t)s2 * plsz;
         const int base = own0 + col.off;
-        int thr[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-        if (P::kFrac) {   // filter thresholds of the column's steps (warp-uniform, L1-resident)
-          const int4 t0 = __ldg((const int4 *)(a.thr + 8 * c)), t1 = __ldg((const int4 *)(a.thr + 8 * c + 4));
-          thr[0] = t0.x; thr[1] = t0.y; thr[2] = t0.z; thr[3] = t0.w; thr[4] = t1.x; thr[5] = t1.y; thr[6] = t1.z; thr[7] = t1.w;
-        }
+        const int *thr = sthr + 8 * c;   // filter thresholds of the column's steps
         if (!slow) {
           p.fast_begin();
           lat_run_col<false, NPAIR>(p, pl, psz, base, a.SX, n, bits, nfb, clr, thr);
@@ -380,6 +391,217 @@ __global__ void __launch_bounds__(MAXT) k_lat_march(const __grid_constant__ LatA
 
 }  // namespace
 
+// ================================================================================================
+// DIRECT variant: no shared-memory staging and no CTA barriers.  One warp owns a row group
+// (32 lanes x 4 rows) at one level and walks ALL stencil columns for it; the neighbour records are
+// read straight from the dense pair arrays with 16-byte loads (a warp reads 512 contiguous bytes per
+// pair; the records of a stencil neighbourhood are shared between the warps of a CTA through L1).
+// Addresses are arithmetic (cell + stencil offset): nothing is read to find a neighbour.
+namespace {
+
+// predicated 16-byte read-only load: no branch, so the four bonds of a step stay in one basic block
+__device__ __forceinline__ void ldg_if(double2 &v, const double2 *ptr, uint32_t pred) {
+  asm("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %3, 0;\n\t@p ld.global.nc.v2.f64 {%0, %1}, [%2];\n\t}"
+      : "+d"(v.x), "+d"(v.y) : "l"(ptr), "r"(pred));
+}
+template <int NPAIR, class E>
+__device__ __forceinline__ void ldg_ent(E &e, const double2 *nb, int64_t npad, int64_t idx) {
+  constexpr int DIMP = sizeof(e.p) / sizeof(double2);
+#pragma unroll
+  for (int k = 0; k < DIMP; ++k) e.p[k] = __ldg(nb + (int64_t)k * npad + idx);
+  if (NPAIR > DIMP) e.g = __ldg(nb + (int64_t)PD_P_AUX * npad + idx);
+}
+template <int NPAIR, class E>
+__device__ __forceinline__ void ldg_ent_if(E &e, const double2 *nb, int64_t npad, int64_t idx, uint32_t pred) {
+  constexpr int DIMP = sizeof(e.p) / sizeof(double2);
+#pragma unroll
+  for (int k = 0; k < DIMP; ++k) ldg_if(e.p[k], nb + (int64_t)k * npad + idx, pred);
+  if (NPAIR > DIMP) ldg_if(e.g, nb + (int64_t)PD_P_AUX * npad + idx, pred);
+}
+
+template <bool MASKED, int NPAIR, class P>
+__device__ __forceinline__ void dir_run_col(P &p, const double2 *nb, int64_t npad, int64_t base, int DX, int n,
+                                            const uint32_t (&bits)[4], const uint32_t (&nfb)[4], uint32_t (&clr)[4],
+                                            const int *thr) {
+  typename P::E S[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) ldg_ent<NPAIR>(S[q], nb, npad, base + (int64_t)q * DX);
+  uint32_t anyp = 0;
+  if (MASKED) anyp = __reduce_or_sync(FULL, bits[0] | (bits[1] << 7) | (bits[2] << 14) | (bits[3] << 21));
+  auto bond = [&](int r, const typename P::E &e, int t) {
+    if (p.template bond<MASKED>(r, e, (bits[r] >> t) & 1u, (nfb[r] >> t) & 1u)) clr[r] |= 1u << t;
+  };
+#pragma unroll
+  for (int t = 0; t < PD_MAXSTEP; ++t) {
+    if (t < n) {
+      const bool live = !MASKED || (anyp & (0x204081u << t)) != 0;   // warp-uniform
+      if (live) bond(0, S[t % 4], t);
+      ldg_ent_if<NPAIR>(S[t % 4], nb, npad, base + (int64_t)(t + 4) * DX, (t + 1 < n) ? 1u : 0u);
+      if (live) {
+        bond(1, S[(t + 1) % 4], t);
+        bond(2, S[(t + 2) % 4], t);
+        bond(3, S[(t + 3) % 4], t);
+      }
+      if (!MASKED && P::kFrac) p.step_end(thr[t]);
+    }
+  }
+}
+
+struct DirArgs {
+  int DX, DY, HX, HY, HZ, PZ;
+  int nxc, nyq, nyq_used;            // x chunks; rgocc stride; row groups along y that can hold nodes
+  int ncol, nw, cy, cz;              // columns; mask words; row groups (y) and levels (z) per CTA
+  int64_t npad;
+  const double2 *nbr;
+  double2 *nbw;
+  uint32_t *mask;
+  const uint32_t *nofail;
+  const uint8_t *rgocc;
+  const uint32_t *flags32;
+  const double *minv;
+  const int32_t *thr;
+  double *v[3];
+  const double *bval[3];
+  double *theta_out;
+  double A, c1, G, s_c, vol_uniform, rrho, dt, gramp;
+  struct Col { int off; uint8_t n, word, bit0, pad; } cols[PD_LAT_MAXCOL];   // off = (dz*DY + dy0)*DX + dx (dense cells)
+};
+
+template <int DIM, bool FORCE, bool FRAC, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) k_lat_direct(const __grid_constant__ DirArgs a) {
+  extern __shared__ __align__(16) unsigned char smraw[];
+  constexpr int NPAIR = FORCE ? DIM + 1 : DIM;
+  using P = typename PolicyOf<DIM, FORCE, FRAC>::type;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
+  // shared: column table, thresholds, per-warp mask words [nwarp][4 words][4 rows][32]
+  DirArgs::Col *scol = (DirArgs::Col *)smraw;
+  int *sthr = (int *)(scol + a.ncol);
+  uint32_t *smk = (uint32_t *)(sthr + (FORCE ? 0 : a.ncol * 8)) + warp * 512;
+  for (int c = tid; c < a.ncol; c += blockDim.x) scol[c] = a.cols[c];
+  if (!FORCE && a.thr)
+    for (int c = tid; c < a.ncol * 8; c += blockDim.x) sthr[c] = a.thr[c];
+  // this warp's row group: (xc, yq, z)
+  const int wy = warp % a.cy, wz = warp / a.cy;
+  const int xc = blockIdx.x, yq = blockIdx.y * a.cy + wy, z = blockIdx.z * a.cz + wz;
+  const bool active = yq < a.nyq_used && z < a.PZ && a.rgocc[((int64_t)z * a.nyq + yq) * a.nxc + xc] != 0;
+  const int64_t i0 = ((int64_t)(z + a.HZ) * a.DY + (yq * 4 + a.HY)) * a.DX + (xc * 32 + lane + a.HX);   // row 0's cell
+  if (active) {
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+      for (int w = 0; w < a.nw; ++w) smk[(w * 4 + r) * 32 + lane] = a.mask[(int64_t)w * a.npad + i0 + (int64_t)r * a.DX];
+  }
+  __syncthreads();   // tables visible (the only CTA barrier)
+  if (!active) return;
+  P p;
+#pragma unroll
+  for (int r = 0; r < 4; ++r) {
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) {
+      const double2 xu = a.nbr[(int64_t)k * a.npad + i0 + (int64_t)r * a.DX];
+      p.xo[r][k] = xu.x;
+      p.uo[r][k] = xu.y;
+    }
+  }
+  if constexpr (FORCE) {
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      const double2 g = a.nbr[(int64_t)PD_P_AUX * a.npad + i0 + (int64_t)r * a.DX];
+      p.gmu_i[r] = g.x;
+      p.cth_i[r] = g.y;
+#pragma unroll
+      for (int k = 0; k < DIM; ++k) p.f[r][k] = 0.0;
+    }
+  } else {
+    p.s_c = a.s_c;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) p.acc[r] = 0.0;
+  }
+  bool dirty = false;
+  for (int c = 0; c < a.ncol; ++c) {
+    const DirArgs::Col col = scol[c];
+    const int n = col.n;
+    const uint32_t nmask = (1u << n) - 1u;
+    uint32_t bits[4], nfb[4] = {0, 0, 0, 0}, clr[4] = {0, 0, 0, 0};
+#pragma unroll
+    for (int r = 0; r < 4; ++r) bits[r] = (smk[(col.word * 4 + r) * 32 + lane] >> col.bit0) & nmask;
+    bool slow = !__all_sync(FULL, (bits[0] & bits[1] & bits[2] & bits[3]) == nmask);
+    const int64_t base = i0 + col.off;
+    const int *thr = sthr + 8 * c;
+    if (!slow) {
+      p.fast_begin();
+      dir_run_col<false, NPAIR>(p, a.nbr, a.npad, base, a.DX, n, bits, nfb, clr, thr);
+      slow = p.fast_failed();
+    }
+    if (slow) {
+      if (P::kFrac && a.nofail) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r) nfb[r] = (a.nofail[(int64_t)col.word * a.npad + i0 + (int64_t)r * a.DX] >> col.bit0) & nmask;
+      }
+      dir_run_col<true, NPAIR>(p, a.nbr, a.npad, base, a.DX, n, bits, nfb, clr, thr);
+      if (P::kFrac) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+          if (clr[r]) { smk[(col.word * 4 + r) * 32 + lane] &= ~(clr[r] << col.bit0); dirty = true; }
+      }
+    }
+  }
+  if (FRAC && __any_sync(FULL, dirty)) {   // broken bits back to HBM
+    if (dirty) {
+#pragma unroll
+      for (int r = 0; r < 4; ++r)
+        for (int w = 0; w < a.nw; ++w) a.mask[(int64_t)w * a.npad + i0 + (int64_t)r * a.DX] = smk[(w * 4 + r) * 32 + lane];
+    }
+  }
+  if constexpr (!FORCE) {
+    double mi[4];
+#pragma unroll
+    for (int r = 0; r < 4; ++r) mi[r] = a.minv[i0 + (int64_t)r * a.DX];
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      const int64_t i = i0 + (int64_t)r * a.DX;
+      const double theta = a.A * mi[r] * (p.acc[r] * a.vol_uniform);   // minv = 0 for phantoms
+      a.nbw[(int64_t)PD_P_AUX * a.npad + i] = make_double2(a.G * mi[r], a.c1 * theta * mi[r]);
+      if (a.theta_out) a.theta_out[i] = theta;
+    }
+  } else {
+    // ---- Eq. 2.11 + boundary dofs (App. B) ----
+    double vk[4][DIM];
+    unsigned fl[4];
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      fl[r] = a.flags32[i0 + (int64_t)r * a.DX];
+#pragma unroll
+      for (int k = 0; k < DIM; ++k) vk[r][k] = a.v[k][i0 + (int64_t)r * a.DX];
+    }
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      if (p.gmu_i[r] == 0.0) continue;   // phantom (a node has m_i > 0)
+      const int64_t i = i0 + (int64_t)r * a.DX;
+#pragma unroll
+      for (int k = 0; k < DIM; ++k) {
+        const double fk = p.f[r][k] * a.vol_uniform;
+        double vv = vk[r][k];
+        double uk = p.uo[r][k];
+        if (fl[r] & (1u << k)) {                       // clamped: u stays, v = 0
+          vv = 0.0;
+        } else if (fl[r] & (8u << k)) {                // prescribed velocity
+          vv = a.bval[k][i];
+          uk = __dadd_rn(uk, __dmul_rn(a.dt, vv));
+        } else {
+          const double bk = (fl[r] & PD_BODY_FORCE) ? a.bval[k][i] : 0.0;
+          const double ac = __dmul_rn(__dadd_rn(fk, __dmul_rn(a.gramp, bk)), a.rrho);   // (f + g b) / rho
+          vv = __dadd_rn(vv, __dmul_rn(a.dt, ac));
+          uk = __dadd_rn(uk, __dmul_rn(a.dt, vv));
+        }
+        a.v[k][i] = vv;
+        a.nbw[(int64_t)k * a.npad + i] = make_double2(p.xo[r][k], uk);
+      }
+    }
+  }
+}
+
+}  // namespace
+
 namespace {
 
 // phi_i = 1 - sum_j rho_ij V_j / sum_j V_j (Eq. 1.31) and the three damage scalars
@@ -462,7 +684,7 @@ size_t lat_make_args(pd_sim *s, LatArgs &a, bool force, int TY, int LZ, int nspl
   a.A = s->A; a.c1 = s->c1; a.G = s->G; a.s_c = s->s_c; a.vol_uniform = s->vol_uniform; a.rrho = 1.0 / s->rho; a.dt = s->dt;
   a.gramp = 1.0;
   if (s->ramp_time > 0.0) a.gramp = std::min(1.0, ((double)s->step * s->dt) / s->ramp_time);
-  return lat_smem(npair, force ? dim : 1, force, a.NP, a.SY, a.SX, TY, nsplit, force ? 4 * dim : 4).total;
+  return lat_smem(npair, force ? dim : 1, force, a.NP, a.SY, a.SX, TY, nsplit, force ? 4 * dim : 4, k).total;
 }
 
 // TY, NSPLIT, LZ: environment overrides (tuning), else the largest configuration that fits
@@ -490,7 +712,7 @@ bool lat_pick(pd_sim *s, LatArgs &a, bool force, int maxthreads, int &TY, int &L
     int nzs = std::max(1, std::min(l.PZ / 6, (592 + ncols - 1) / ncols));
     LZ = (l.PZ + nzs - 1) / nzs;
   }
-  LZ = std::max(1, std::min(LZ, l.PZ));
+  LZ = std::max(1, std::min(std::min(LZ, 64), l.PZ));   // (a 64-bit activity mask per CTA)
   smem = lat_make_args(s, a, force, TY, LZ, nsplit);
   return true;
 }
@@ -571,11 +793,105 @@ LatPrepared *lat_prepare(pd_sim *s, bool force) {
   return pp;
 }
 
+// ---- direct variant: arguments (cached next to the marching ones) and launch ----
+struct DirPrepared {
+  DirArgs a;
+  size_t smem = 0;
+  dim3 grid, block;
+};
+
+bool lat_use_direct() {
+  static int mode = -1;
+  if (mode < 0) {
+    const char *e = getenv("PD_LAT_KERNEL");   // "march" selects the shared-memory marching kernels
+    mode = (e && !strcmp(e, "march")) ? 0 : 1;
+  }
+  return mode == 1;
+}
+
+DirPrepared *dir_prepare(pd_sim *s, bool force) {
+  PdLattice &l = s->lat;
+  static_assert(sizeof(void *) == 8, "");
+  void *&slot = l.cache[2 + (force ? 1 : 0)];
+  if (slot) return (DirPrepared *)slot;
+  DirPrepared *pp = new DirPrepared();
+  slot = pp;
+  DirArgs &a = pp->a;
+  a.DX = l.DX; a.DY = l.DY; a.HX = l.HX; a.HY = l.HY; a.HZ = l.HZ; a.PZ = l.PZ;
+  a.nxc = l.PX / 32; a.nyq = (l.PY + 8) / 4; a.nyq_used = l.PY / 4;
+  a.ncol = l.ncol; a.nw = l.nw;
+  a.cy = std::max(1, std::min(env_int(force ? "PD_DIR_FRC_CY" : "PD_DIR_DIL_CY", 2), 4));
+  a.cz = s->dim == 3 ? std::max(1, std::min(env_int(force ? "PD_DIR_FRC_CZ" : "PD_DIR_DIL_CZ", 2), 4)) : 1;
+  while (a.cy * a.cz > 4) { if (a.cz > 1) --a.cz; else --a.cy; }   // 128 threads per CTA
+  a.npad = s->npad;
+  for (int c = 0; c < l.ncol; ++c) {
+    const PdLatCol &src = l.cols[c];
+    a.cols[c].off = (src.dz * l.DY + src.dy0) * l.DX + src.dx;
+    a.cols[c].n = src.n; a.cols[c].word = src.word; a.cols[c].bit0 = src.bit0; a.cols[c].pad = 0;
+  }
+  a.mask = l.mask; a.nofail = l.nofail; a.rgocc = l.rgocc; a.flags32 = l.flags32; a.minv = s->minv;
+  for (int q = 0; q < 3; ++q) { a.v[q] = s->v[q]; a.bval[q] = s->bval[q]; }
+  a.theta_out = nullptr;
+  a.A = s->A; a.c1 = s->c1; a.G = s->G; a.s_c = s->s_c; a.vol_uniform = s->vol_uniform; a.rrho = 1.0 / s->rho; a.dt = s->dt;
+  a.gramp = 1.0;
+  a.thr = nullptr;
+  if (!force) {   // break-test filter thresholds (pd_bond.cuh, DilPolicy FILT): high word of s_c * min ||xi||^2, a shade low
+    std::vector<int32_t> h((size_t)PD_LAT_MAXCOL * 8, 0);
+    for (int c = 0; c < l.ncol; ++c)
+      for (int t = 0; t < l.cols[c].n; ++t) {
+        const double thr = s->s_c * l.r2lb[l.cols[c].word * 32 + l.cols[c].bit0 + t] * (1.0 - 1.0 / 1099511627776.0);
+        long long bits;
+        memcpy(&bits, &thr, 8);
+        h[(size_t)c * 8 + t] = (int32_t)(bits >> 32);
+      }
+    if (!l.thr_dir) l.thr_dir = (int32_t *)pdi::dev_alloc(s, sizeof(int32_t) * h.size());
+    if (l.thr_dir) {
+      cudaMemcpyAsync(l.thr_dir, h.data(), sizeof(int32_t) * h.size(), cudaMemcpyHostToDevice, s->stream);
+      cudaStreamSynchronize(s->stream);
+    }
+    a.thr = l.thr_dir;
+  }
+  const int nwarp = a.cy * a.cz;
+  pp->smem = (size_t)l.ncol * 8 + (force ? 0 : (size_t)l.ncol * 32) + (size_t)nwarp * 2048;
+  pp->block = dim3((unsigned)(nwarp * 32));
+  pp->grid = dim3((unsigned)a.nxc, (unsigned)((a.nyq_used + a.cy - 1) / a.cy), (unsigned)((l.PZ + a.cz - 1) / a.cz));
+  return pp;
+}
+
+int dir_launch(pd_sim *s, bool force, double *theta_out, bool frac) {
+  DirPrepared *pp = dir_prepare(s, force);
+  DirArgs &a = pp->a;
+  a.nbr = s->nb[s->cur]; a.nbw = s->nb[force ? s->cur ^ 1 : s->cur];
+  a.theta_out = theta_out;
+  if (force) {
+    a.gramp = 1.0;
+    if (s->ramp_time > 0.0) a.gramp = std::min(1.0, ((double)s->step * s->dt) / s->ramp_time);
+  } else if (frac && !a.thr) {
+    pdi::set_error("device allocation failed");
+    return PD_ERR_ALLOC;
+  }
+  if (force) {
+    if (s->dim == 2) k_lat_direct<2, true, false, 128, 2><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);
+    else k_lat_direct<3, true, false, 128, 2><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);
+  } else if (frac) {
+    if (s->dim == 2) k_lat_direct<2, false, true, 128, 3><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);
+    else k_lat_direct<3, false, true, 128, 3><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);
+  } else {
+    if (s->dim == 2) k_lat_direct<2, false, false, 128, 3><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);
+    else k_lat_direct<3, false, false, 128, 3><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);
+  }
+  return PD_OK;
+}
+
 }  // namespace
 
 namespace pdi {
 
 void lat_free_cache(pd_sim *s) {
+  for (int q = 2; q < 4; ++q) {
+    delete (DirPrepared *)s->lat.cache[q];
+    s->lat.cache[q] = nullptr;
+  }
   for (int q = 0; q < 2; ++q) {
     delete (LatPrepared *)s->lat.cache[q];
     s->lat.cache[q] = nullptr;
@@ -583,6 +899,7 @@ void lat_free_cache(pd_sim *s) {
 }
 
 int lat_launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
+  if (lat_use_direct()) return dir_launch(s, false, theta_out, do_break && s->fracture);
   LatPrepared *pp = lat_prepare(s, false);
   if (!pp->ok) { set_error("lattice plane ring does not fit shared memory"); return PD_ERR_LIMIT; }
   LatArgs &a = pp->a;
@@ -596,6 +913,7 @@ int lat_launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
 }
 
 int lat_launch_force_update(pd_sim *s) {
+  if (lat_use_direct()) return dir_launch(s, true, nullptr, false);
   LatPrepared *pp = lat_prepare(s, true);
   if (!pp->ok) { set_error("lattice plane ring does not fit shared memory"); return PD_ERR_LIMIT; }
   LatArgs &a = pp->a;
