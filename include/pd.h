@@ -97,8 +97,8 @@ typedef struct {
 /*
  * pd_create -- pre-processing, run once.  Builds on the GPU: the cell list, the
  * locality-sorted node order, the family H_i = { j != i : ||x_j - x_i|| <= horizon } (inclusive,
- * PAPER.md:121-125) as a sliced-ELL neighbour layout with one intact/broken bit per directed
- * bond (Eq. 1.30), the weighted volume m_i = sum_j ||xi_ij||^2 V_j (Eq. 1.9, w = 1)
+ * PAPER.md:121-125) with one intact/broken bit per directed bond (Eq. 1.30) -- as stencil bit masks
+ * over a dense cell array when the body is a lattice, else as a sliced-ELL neighbour list --, the weighted volume m_i = sum_j ||xi_ij||^2 V_j (Eq. 1.9, w = 1)
  * and the family volume sum_j V_j (denominator of Eq. 1.31), both over the full geometric
  * family and never updated; clears the bits of the pre-cut pairs (both directions).
  *   coords  dim*n AoS reference positions; volumes n nodal volumes V_i (> 0)
@@ -146,9 +146,11 @@ PD_API int pd_get_bond_mask(pd_sim *sim, int64_t *rowptr, int32_t *col, uint8_t 
  * dilatation theta_i of the current displacement (Eq. 1.6). */
 PD_API int pd_get_node_fields(pd_sim *sim, double *m, double *theta);
 
-/* layout/launch facts for the roofline report: counts[0]=n, [1]=n padded, [2]=Z directed bonds,
- * [3]=stored neighbour slots (Z + padding), [4]=kernel launches issued by pd_step so far,
- * [5]=bytes of device memory held, [6]=1 if volumes are uniform, [7]=fine cells per horizon. */
+/* layout/launch facts for the roofline report: counts[0]=n, [1]=n padded (array length incl. phantoms),
+ * [2]=Z directed bonds, [3]=stored neighbour-index slots (0 in the lattice layout, which stores none),
+ * [4]=kernel launches issued by pd_step so far, [5]=bytes of device memory held, [6]=1 if volumes are
+ * uniform, [7]=layout: 0 = windowed sliced ELL (any point cloud), 1 = dense lattice / direct kernels,
+ * 2 = dense lattice / shared-memory marching kernels. */
 PD_API int pd_get_layout(pd_sim *sim, int64_t counts[8]);
 
 /* measurement aid for the roofline report: like pd_step, but brackets every kernel launch with

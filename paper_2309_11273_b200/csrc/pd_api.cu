@@ -328,7 +328,8 @@ int pd_get_bond_mask(pd_sim *s, int64_t *rowptr, int32_t *col, uint8_t *intact) 
 int pd_get_layout(pd_sim *s, int64_t counts[8]) {
   if (!s || !counts) { pdi::set_error("null argument"); return PD_ERR_ARG; }
   counts[0] = s->n; counts[1] = s->npad; counts[2] = s->Z; counts[3] = s->nentries * 32;
-  counts[4] = s->launches; counts[5] = (int64_t)s->bytes_held; counts[6] = s->uniform_v ? 1 : 0; counts[7] = s->kdiv;
+  counts[4] = s->launches; counts[5] = (int64_t)s->bytes_held; counts[6] = s->uniform_v ? 1 : 0;
+  counts[7] = s->lat.on ? 1 + s->lat.kernel : 0;
   return PD_OK;
 }
 

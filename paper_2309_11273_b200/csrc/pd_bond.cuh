@@ -101,6 +101,63 @@ struct DilPolicy {
     }
     return brk;
   }
+
+  // ---- staged form of one STEP (the R bonds of the R rows with R records), written phase by phase
+  // over the rows so that every instruction has R - 1 independent ones between it and its consumer.
+  // Same arithmetic, operand by operand, as bond().
+  double xi_[R][DIM], eta_[R][DIM];
+  __device__ __forceinline__ void diffs(int r, const E &e) {
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) {
+      xi_[r][k] = e.p[k].x - xo[r][k];
+      eta_[r][k] = e.p[k].y - uo[r][k];
+    }
+  }
+  // in / nofail: bit r = row r (MASKED only); returns the rows whose bond breaks now
+  template <bool MASKED>
+  __device__ __forceinline__ uint32_t finish(uint32_t in, uint32_t nofail) {
+    static_assert(UNIV, "staged form: uniform volume only");
+    double dot[R], r2[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) dot[r] = __dmul_rn(xi_[r][0], eta_[r][0]);
+    constexpr bool EXACT = FRAC && (MASKED || !FILT);
+    if (EXACT) {
+#pragma unroll
+      for (int r = 0; r < R; ++r) r2[r] = __dmul_rn(xi_[r][0], xi_[r][0]);
+    }
+#pragma unroll
+    for (int k = 1; k < DIM; ++k) {
+#pragma unroll
+      for (int r = 0; r < R; ++r) dot[r] = fma(xi_[r][k], eta_[r][k], dot[r]);
+      if (EXACT) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) r2[r] = fma(xi_[r][k], xi_[r][k], r2[r]);
+      }
+    }
+    uint32_t brk = 0;
+    if (!MASKED) in = (1u << R) - 1u;
+    if (FRAC && FILT && !MASKED) {
+#pragma unroll
+      for (int r = 0; r < R; ++r) mxhi = max(mxhi, __double2hiint(dot[r]));
+    } else if (FRAC) {
+      double t[R];
+#pragma unroll
+      for (int r = 0; r < R; ++r) t[r] = fma(-s_c, r2[r], dot[r]);
+      if (MASKED) {
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+          if (((in >> r) & 1u) && __double2hiint(t[r]) >= 0 && !((nofail >> r) & 1u)) brk |= 1u << r;
+        in &= ~brk;
+      } else {
+#pragma unroll
+        for (int r = 0; r < R; ++r) sg &= __double2hiint(t[r]);
+      }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+      if ((in >> r) & 1u) acc[r] += dot[r];
+    return brk;
+  }
 };
 
 // 1/x seed: MUFU.RCP64H (relative error about 2^-20)
@@ -143,6 +200,53 @@ struct ForcePolicy {
       for (int k = 0; k < DIM; ++k) f[r][k] = fma(t, xi[k], f[r][k]);
     }
     return false;
+  }
+
+  // ---- staged form of one step (see DilPolicy): same arithmetic as bond(), phase by phase over the rows
+  double xi_[R][DIM], eta_[R][DIM], gs_[R], cs_[R];
+  __device__ __forceinline__ void diffs(int r, const E &e) {
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) {
+      xi_[r][k] = e.p[k].x - xo[r][k];
+      eta_[r][k] = e.p[k].y - uo[r][k];
+    }
+    gs_[r] = gmu_i[r] + e.g.x;
+    cs_[r] = cth_i[r] + e.g.y;
+  }
+  template <bool MASKED>
+  __device__ __forceinline__ uint32_t finish(uint32_t in, uint32_t) {
+    static_assert(UNIV, "staged form: uniform volume only");
+    double dot[R], r2[R], y[R], err[R], q[R], t[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) r2[r] = __dmul_rn(xi_[r][0], xi_[r][0]);
+#pragma unroll
+    for (int r = 0; r < R; ++r) dot[r] = __dmul_rn(xi_[r][0], eta_[r][0]);
+#pragma unroll
+    for (int k = 1; k < DIM; ++k) {
+#pragma unroll
+      for (int r = 0; r < R; ++r) r2[r] = fma(xi_[r][k], xi_[r][k], r2[r]);
+#pragma unroll
+      for (int r = 0; r < R; ++r) dot[r] = fma(xi_[r][k], eta_[r][k], dot[r]);
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) y[r] = rcp_seed(r2[r]);
+#pragma unroll
+    for (int r = 0; r < R; ++r) err[r] = fma(-r2[r], y[r], 1.0);
+#pragma unroll
+    for (int r = 0; r < R; ++r) q[r] = __dmul_rn(dot[r], y[r]);
+#pragma unroll
+    for (int r = 0; r < R; ++r) err[r] = fma(err[r], err[r], err[r]);
+#pragma unroll
+    for (int r = 0; r < R; ++r) q[r] = fma(q[r], err[r], q[r]);
+#pragma unroll
+    for (int r = 0; r < R; ++r) t[r] = fma(gs_[r], q[r], cs_[r]);
+    if (!MASKED) in = (1u << R) - 1u;   // rho_ij
+#pragma unroll
+    for (int k = 0; k < DIM; ++k)
+#pragma unroll
+      for (int r = 0; r < R; ++r)
+        if ((in >> r) & 1u) f[r][k] = fma(t[r], xi_[r][k], f[r][k]);
+    return 0u;
   }
 };
 

@@ -110,6 +110,7 @@ struct PdGrid {
 };
 struct PdLattice {
   bool on = false;
+  int kernel = 0;                  // 0: direct kernels (default), 1: shared-memory marching kernels (PD_LAT_KERNEL=march)
   int DX = 0, DY = 0, DZ = 0;      // dense dims incl. margins
   int HX = 0, HY = 0, HZ = 0;      // margins = stencil radius per axis
   int PX = 0, PY = 0, PZ = 0;      // padded cell counts (PX multiple of 32, PY of 4)

@@ -263,6 +263,8 @@ int build_lattice(pd_sim *s, const PdGrid &g, const double *coords, const double
   l.on = false;
   if (!s->uniform_v) return 0;
   if (const char *env = getenv("PD_FORCE_GENERIC")) { if (atoi(env)) return 0; }
+  l.kernel = 0;
+  if (const char *env = getenv("PD_LAT_KERNEL")) { if (!strcmp(env, "march")) l.kernel = 1; }
   const double ncell = (double)g.nc[0] * g.nc[1] * g.nc[2];
   if ((double)n < 0.2 * ncell) return 0;                      // too sparse for a dense array
   std::vector<void *> scratch;

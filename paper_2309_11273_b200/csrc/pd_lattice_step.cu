@@ -404,28 +404,29 @@ __device__ __forceinline__ void ldg_if(double2 &v, const double2 *ptr, uint32_t 
   asm("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %3, 0;\n\t@p ld.global.nc.v2.f64 {%0, %1}, [%2];\n\t}"
       : "+d"(v.x), "+d"(v.y) : "l"(ptr), "r"(pred));
 }
+// a record = NPAIR pairs; pk[k] points at pair k of the warp's own row-0 cell, off is the (32-bit) cell offset
 template <int NPAIR, class E>
-__device__ __forceinline__ void ldg_ent(E &e, const double2 *nb, int64_t npad, int64_t idx) {
+__device__ __forceinline__ void ldg_ent(E &e, const double2 *const (&pk)[NPAIR], int off) {
   constexpr int DIMP = sizeof(e.p) / sizeof(double2);
 #pragma unroll
-  for (int k = 0; k < DIMP; ++k) e.p[k] = __ldg(nb + (int64_t)k * npad + idx);
-  if (NPAIR > DIMP) e.g = __ldg(nb + (int64_t)PD_P_AUX * npad + idx);
+  for (int k = 0; k < DIMP; ++k) e.p[k] = __ldg(pk[k] + off);
+  if (NPAIR > DIMP) e.g = __ldg(pk[DIMP] + off);
 }
 template <int NPAIR, class E>
-__device__ __forceinline__ void ldg_ent_if(E &e, const double2 *nb, int64_t npad, int64_t idx, uint32_t pred) {
+__device__ __forceinline__ void ldg_ent_if(E &e, const double2 *const (&pk)[NPAIR], int off, uint32_t pred) {
   constexpr int DIMP = sizeof(e.p) / sizeof(double2);
 #pragma unroll
-  for (int k = 0; k < DIMP; ++k) ldg_if(e.p[k], nb + (int64_t)k * npad + idx, pred);
-  if (NPAIR > DIMP) ldg_if(e.g, nb + (int64_t)PD_P_AUX * npad + idx, pred);
+  for (int k = 0; k < DIMP; ++k) ldg_if(e.p[k], pk[k] + off, pred);
+  if (NPAIR > DIMP) ldg_if(e.g, pk[DIMP] + off, pred);
 }
 
-template <bool MASKED, int NPAIR, class P>
-__device__ __forceinline__ void dir_run_col(P &p, const double2 *nb, int64_t npad, int64_t base, int DX, int n,
+template <bool MASKED, bool STAGED, int NPAIR, class P>
+__device__ __forceinline__ void dir_run_col(P &p, const double2 *const (&pk)[NPAIR], int base, int DX, int n,
                                             const uint32_t (&bits)[4], const uint32_t (&nfb)[4], uint32_t (&clr)[4],
                                             const int *thr) {
   typename P::E S[4];
 #pragma unroll
-  for (int q = 0; q < 4; ++q) ldg_ent<NPAIR>(S[q], nb, npad, base + (int64_t)q * DX);
+  for (int q = 0; q < 4; ++q) ldg_ent<NPAIR>(S[q], pk, base + q * DX);
   uint32_t anyp = 0;
   if (MASKED) anyp = __reduce_or_sync(FULL, bits[0] | (bits[1] << 7) | (bits[2] << 14) | (bits[3] << 21));
   auto bond = [&](int r, const typename P::E &e, int t) {
@@ -435,12 +436,34 @@ __device__ __forceinline__ void dir_run_col(P &p, const double2 *nb, int64_t npa
   for (int t = 0; t < PD_MAXSTEP; ++t) {
     if (t < n) {
       const bool live = !MASKED || (anyp & (0x204081u << t)) != 0;   // warp-uniform
-      if (live) bond(0, S[t % 4], t);
-      ldg_ent_if<NPAIR>(S[t % 4], nb, npad, base + (int64_t)(t + 4) * DX, (t + 1 < n) ? 1u : 0u);
-      if (live) {
-        bond(1, S[(t + 1) % 4], t);
-        bond(2, S[(t + 2) % 4], t);
-        bond(3, S[(t + 3) % 4], t);
+      if (STAGED) {
+        // differences of the 4 rows first (row 0 frees its slot for the next record), then the products
+        // phase by phase over the rows (pd_bond.cuh, finish)
+        if (live) p.diffs(0, S[t % 4]);
+        ldg_ent_if<NPAIR>(S[t % 4], pk, base + (t + 4) * DX, (t + 1 < n) ? 1u : 0u);
+        if (live) {
+          p.diffs(1, S[(t + 1) % 4]);
+          p.diffs(2, S[(t + 2) % 4]);
+          p.diffs(3, S[(t + 3) % 4]);
+          uint32_t in4 = 15u, nf4 = 0u;
+          if (MASKED) {
+            in4 = ((bits[0] >> t) & 1u) | (((bits[1] >> t) & 1u) << 1) | (((bits[2] >> t) & 1u) << 2) | (((bits[3] >> t) & 1u) << 3);
+            nf4 = ((nfb[0] >> t) & 1u) | (((nfb[1] >> t) & 1u) << 1) | (((nfb[2] >> t) & 1u) << 2) | (((nfb[3] >> t) & 1u) << 3);
+          }
+          const uint32_t brk = p.template finish<MASKED>(in4, nf4);
+          if (MASKED && P::kFrac) {
+#pragma unroll
+            for (int r = 0; r < 4; ++r) clr[r] |= ((brk >> r) & 1u) << t;
+          }
+        }
+      } else {
+        if (live) bond(0, S[t % 4], t);
+        ldg_ent_if<NPAIR>(S[t % 4], pk, base + (t + 4) * DX, (t + 1 < n) ? 1u : 0u);   // record t+4: row 3 of step t+1
+        if (live) {
+          bond(1, S[(t + 1) % 4], t);
+          bond(2, S[(t + 2) % 4], t);
+          bond(3, S[(t + 3) % 4], t);
+        }
       }
       if (!MASKED && P::kFrac) p.step_end(thr[t]);
     }
@@ -467,7 +490,7 @@ struct DirArgs {
   struct Col { int off; uint8_t n, word, bit0, pad; } cols[PD_LAT_MAXCOL];   // off = (dz*DY + dy0)*DX + dx (dense cells)
 };
 
-template <int DIM, bool FORCE, bool FRAC, int MAXT, int MINB>
+template <int DIM, bool FORCE, bool FRAC, int MAXT, int MINB, bool STAGED>
 __global__ void __launch_bounds__(MAXT, MINB) k_lat_direct(const __grid_constant__ DirArgs a) {
   extern __shared__ __align__(16) unsigned char smraw[];
   constexpr int NPAIR = FORCE ? DIM + 1 : DIM;
@@ -516,6 +539,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_lat_direct(const __grid_constant
 #pragma unroll
     for (int r = 0; r < 4; ++r) p.acc[r] = 0.0;
   }
+  const double2 *pk[NPAIR];   // pair k of the warp's own row-0 cell: a record is pk[k] + (32-bit cell offset)
+#pragma unroll
+  for (int k = 0; k < NPAIR; ++k) pk[k] = a.nbr + (int64_t)(k < DIM ? k : PD_P_AUX) * a.npad + i0;
   bool dirty = false;
   for (int c = 0; c < a.ncol; ++c) {
     const DirArgs::Col col = scol[c];
@@ -525,11 +551,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_lat_direct(const __grid_constant
 #pragma unroll
     for (int r = 0; r < 4; ++r) bits[r] = (smk[(col.word * 4 + r) * 32 + lane] >> col.bit0) & nmask;
     bool slow = !__all_sync(FULL, (bits[0] & bits[1] & bits[2] & bits[3]) == nmask);
-    const int64_t base = i0 + col.off;
+    const int base = col.off;
     const int *thr = sthr + 8 * c;
     if (!slow) {
       p.fast_begin();
-      dir_run_col<false, NPAIR>(p, a.nbr, a.npad, base, a.DX, n, bits, nfb, clr, thr);
+      dir_run_col<false, STAGED, NPAIR>(p, pk, base, a.DX, n, bits, nfb, clr, thr);
       slow = p.fast_failed();
     }
     if (slow) {
@@ -537,7 +563,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_lat_direct(const __grid_constant
 #pragma unroll
         for (int r = 0; r < 4; ++r) nfb[r] = (a.nofail[(int64_t)col.word * a.npad + i0 + (int64_t)r * a.DX] >> col.bit0) & nmask;
       }
-      dir_run_col<true, NPAIR>(p, a.nbr, a.npad, base, a.DX, n, bits, nfb, clr, thr);
+      dir_run_col<true, STAGED, NPAIR>(p, pk, base, a.DX, n, bits, nfb, clr, thr);
       if (P::kFrac) {
 #pragma unroll
         for (int r = 0; r < 4; ++r)
@@ -800,15 +826,6 @@ struct DirPrepared {
   dim3 grid, block;
 };
 
-bool lat_use_direct() {
-  static int mode = -1;
-  if (mode < 0) {
-    const char *e = getenv("PD_LAT_KERNEL");   // "march" selects the shared-memory marching kernels
-    mode = (e && !strcmp(e, "march")) ? 0 : 1;
-  }
-  return mode == 1;
-}
-
 DirPrepared *dir_prepare(pd_sim *s, bool force) {
   PdLattice &l = s->lat;
   static_assert(sizeof(void *) == 8, "");
@@ -870,16 +887,20 @@ int dir_launch(pd_sim *s, bool force, double *theta_out, bool frac) {
     pdi::set_error("device allocation failed");
     return PD_ERR_ALLOC;
   }
+  static const int staged = env_int("PD_DIR_STAGED", 2);   // bit 0: dilatation, bit 1: force (phase-ordered step, pd_bond.cuh)
+#define DIR_LAUNCH(DIM_, FORCE_, FRAC_, MINB_, ST_)                                                                      \
+  do {                                                                                                                   \
+    if (ST_) k_lat_direct<DIM_, FORCE_, FRAC_, 128, MINB_, true><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);       \
+    else k_lat_direct<DIM_, FORCE_, FRAC_, 128, MINB_, false><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);          \
+  } while (0)
   if (force) {
-    if (s->dim == 2) k_lat_direct<2, true, false, 128, 2><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);
-    else k_lat_direct<3, true, false, 128, 2><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);
+    if (s->dim == 2) DIR_LAUNCH(2, true, false, 2, staged & 2); else DIR_LAUNCH(3, true, false, 2, staged & 2);
   } else if (frac) {
-    if (s->dim == 2) k_lat_direct<2, false, true, 128, 3><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);
-    else k_lat_direct<3, false, true, 128, 3><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);
+    if (s->dim == 2) DIR_LAUNCH(2, false, true, 3, staged & 1); else DIR_LAUNCH(3, false, true, 3, staged & 1);
   } else {
-    if (s->dim == 2) k_lat_direct<2, false, false, 128, 3><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);
-    else k_lat_direct<3, false, false, 128, 3><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);
+    if (s->dim == 2) DIR_LAUNCH(2, false, false, 3, staged & 1); else DIR_LAUNCH(3, false, false, 3, staged & 1);
   }
+#undef DIR_LAUNCH
   return PD_OK;
 }
 
@@ -899,7 +920,7 @@ void lat_free_cache(pd_sim *s) {
 }
 
 int lat_launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
-  if (lat_use_direct()) return dir_launch(s, false, theta_out, do_break && s->fracture);
+  if (s->lat.kernel == 0) return dir_launch(s, false, theta_out, do_break && s->fracture);
   LatPrepared *pp = lat_prepare(s, false);
   if (!pp->ok) { set_error("lattice plane ring does not fit shared memory"); return PD_ERR_LIMIT; }
   LatArgs &a = pp->a;
@@ -913,7 +934,7 @@ int lat_launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
 }
 
 int lat_launch_force_update(pd_sim *s) {
-  if (lat_use_direct()) return dir_launch(s, true, nullptr, false);
+  if (s->lat.kernel == 0) return dir_launch(s, true, nullptr, false);
   LatPrepared *pp = lat_prepare(s, true);
   if (!pp->ok) { set_error("lattice plane ring does not fit shared memory"); return PD_ERR_LIMIT; }
   LatArgs &a = pp->a;

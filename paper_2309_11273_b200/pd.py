@@ -220,7 +220,7 @@ class Sim:
         c = (C.c_int64 * 8)()
         self._ck(self.lib.pd_get_layout(self.h, C.addressof(c)))
         keys = ["n", "n_padded", "n_directed_bonds", "stored_slots", "step_launches", "device_bytes",
-                "uniform_volume", "cells_per_horizon"]
+                "uniform_volume", "layout"]
         return dict(zip(keys, [int(x) for x in c]))
 
     def destroy(self):

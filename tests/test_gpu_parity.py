@@ -12,6 +12,24 @@ pytestmark = pytest.mark.gpu
 
 TOL = 1e-10
 
+# the three code paths of the library: the layout is chosen inside pd_create; the
+# environment switches exist for exactly this purpose (and for profiling)
+LAYOUTS = {
+    "lattice_direct": ({}, 1),
+    "lattice_march": ({"PD_LAT_KERNEL": "march"}, 2),
+    "sliced_ell": ({"PD_FORCE_GENERIC": "1"}, 0),
+}
+
+
+@pytest.fixture(params=list(LAYOUTS))
+def layout(request, monkeypatch):
+    env, code = LAYOUTS[request.param]
+    for k in ("PD_LAT_KERNEL", "PD_FORCE_GENERIC"):
+        monkeypatch.delenv(k, raising=False)
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    return code
+
 
 def _oracle(wl):
     from oracle.pd_oracle import PDOracle
@@ -47,9 +65,10 @@ def _small_cases():
 
 
 @pytest.mark.parametrize("name", ["config1_full", "config4_small"])
-def test_no_fracture_trajectory(name):
+def test_no_fracture_trajectory(name, layout):
     wl, nsteps = _small_cases()[name]
     sim, o = _sim(wl), _oracle(wl)
+    assert sim.get_layout()["layout"] == layout
     # pre-processing parity: family sizes, m, theta of the initial field
     rp = sim.get_bond_mask(rows_only=True)
     assert np.array_equal(rp, o.rowptr)
@@ -67,9 +86,10 @@ def test_no_fracture_trajectory(name):
 
 
 @pytest.mark.parametrize("name", ["config2_small", "config3_small", "config5_small"])
-def test_fracture_broken_sets(name):
+def test_fracture_broken_sets(name, layout):
     wl, nsteps = _small_cases()[name]
     sim, o = _sim(wl), _oracle(wl)
+    assert sim.get_layout()["layout"] == layout
     b0, rp, col = _broken_set(sim)
     assert np.array_equal(rp, o.rowptr)
     assert b0 == o.broken_set() and len(b0) == 2 * len(wl.precut)
@@ -152,4 +172,41 @@ def test_edge_cases_and_errors():
                  precut=np.zeros((0, 2), np.int32))
     sim.step(0)
     assert sim.get_stats()["step"] == 0 and sim.get_stats()["n_directed_bonds"] == 2
+    sim.destroy()
+
+
+def test_point_cloud_general_layout():
+    """a random cloud (cells with 0, 1 or several nodes): the sliced-ELL layout with its FLAT segments;
+    also a lattice whose stencil exceeds the lattice layout's limits must fall back by itself"""
+    from paper_2309_11273_b200 import pd
+    from oracle.pd_oracle import PDOracle
+    rng = np.random.default_rng(5)
+    n = 3000
+    x = rng.uniform(0.0, 1.0, (n, 3)) * np.array([1.0, 0.6, 0.4])
+    kw = dict(dim=3, mode=0, E=3.0, nu=0.25, rho=1.5, dt=2e-3)
+    u0 = 1e-4 * np.sin(3.0 * x[:, [1, 2, 0]])
+    sim = pd.Sim(x, np.full(n, 1.0 / n), 0.16, **kw, u0=u0)
+    assert sim.get_layout()["layout"] == 0
+    o = PDOracle(x, np.full(n, 1.0 / n), 0.16, **kw, flags=None, value=None, precut=None, u0=u0, v0=None)
+    assert np.array_equal(sim.get_bond_mask(rows_only=True), o.rowptr)
+    sim.step(40); o.step(40)
+    assert _rel(sim.get_u(), o.u) <= TOL and _rel(sim.get_v(), o.v) <= TOL
+    sim.destroy()
+
+
+def test_full_size_config5p_sampled():
+    """BASELINE-size workload (config 5', 1 257 600 nodes) in the launch configuration bench.py times:
+    a few steps against the oracle -- every node for u and v, the complete broken-bond set, damage."""
+    from paper_2309_11273_b200 import workloads as W
+    wl = W.CONFIGS["config5p"]()
+    sim, o = _sim(wl), _oracle(wl)
+    assert sim.get_layout()["layout"] == 1
+    assert sim.get_stats()["n_directed_bonds"] == o.Z
+    sim.step(3); o.step(3)
+    assert _rel(sim.get_u(), o.u) <= TOL and _rel(sim.get_v(), o.v) <= TOL
+    st = sim.get_stats()
+    assert st["n_broken_directed"] == len(o.broken_set()) == 2 * len(wl.precut)
+    rng = np.random.default_rng(0)
+    idx = rng.integers(0, wl.n, 2000)
+    assert np.allclose(sim.get_damage()[idx], o.damage()[idx], rtol=0, atol=1e-12)
     sim.destroy()
