@@ -4,8 +4,8 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config5|config5p|config4|config3|config2|config1]
     python bench.py --impl reference ...      # the CPU oracle as it stands, on the host cores
 
-A "step" is one pass of the whole hot path (dilatation(+break) kernel, force+update kernel) over
-the workload.  Metric (BASELINE.json): node-steps/s, FP64; bond-updates/s and the HBM roofline of
+A "step" is one pass of the whole hot path (dilatation(+break) kernel, force+update kernel: 2 launches)
+over the workload.  Metric (BASELINE.json): node-steps/s, FP64; bond-updates/s and the HBM roofline of
 the dominant kernel are in the same JSON line.  Default workload = config 5 (3D notched cylinder,
 3.144 M nodes, the config the >=60 %-of-HBM-roofline target is quoted on).
 
@@ -237,6 +237,13 @@ def main():
     peak = float(peaks.get("hbm_gbs", 6650.0))
     peak_kind = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
     b_dil, b_frc = byte_model(n, z, wl.dim, fracture)
+    traffic = {}
+    try:   # DRAM bytes per launch of the two kernels from the committed ncu capture (profiles/r01c_direct_kernels.md)
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "r01c_traffic.json"))).get(args.workload, {})
+    except Exception:
+        pass
+    if lay.get("layout") != 1:
+        traffic = {}   # the capture is of the default (lattice / direct) kernels
     t_dil, t_frc = kd / nk * 1e-3, kf / nk * 1e-3
     dom = ("k_force_update", b_frc, t_frc) if t_frc >= t_dil else ("k_dilatation", b_dil, t_dil)
     achieved = dom[1] / dom[2] / 1e9
@@ -253,10 +260,16 @@ def main():
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": {"bound": "hbm", "kernel": dom[0], "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": None, "peak_kind": peak_kind,
+                     "frac": achieved / peak, "traffic": traffic.get(dom[0]), "peak_kind": peak_kind,
                      "algorithmic_bytes_per_launch": dom[1], "kernel_ms": dom[2] * 1e3},
         "kernels": {"k_dilatation": {"ms": t_dil * 1e3, "algorithmic_bytes": b_dil, "GBps": b_dil / t_dil / 1e9},
                     "k_force_update": {"ms": t_frc * 1e3, "algorithmic_bytes": b_frc, "GBps": b_frc / t_frc / 1e9}},
+        # co-limiter: FP64 instructions the arithmetic of the method needs per directed bond
+        # (10 dilatation [14 with the exact break test], 22 force) against 148 SM x 64 FP64 lanes x 1.965 GHz
+        "fp64_roofline": {"bound": "alu", "kernel": "k_force_update", "achieved": 22.0 * z / t_frc / 1e12,
+                          "peak": 148 * 64 * 1.965e9 / 1e12, "unit": "T FP64 instr/s",
+                          "frac": 22.0 * z / t_frc / (148 * 64 * 1.965e9),
+                          "step_frac": (10.0 + 22.0) * z / step_s / (148 * 64 * 1.965e9)},
         "step_roofline": {"algorithmic_bytes_per_step_B2": b_dil + b_frc, "achieved_GBps": (b_dil + b_frc) / step_s / 1e9,
                           "frac_of_peak": (b_dil + b_frc) / step_s / 1e9 / peak, "frac_of_8TBps_nominal":
                           (b_dil + b_frc) / step_s / 8e12},
@@ -266,7 +279,7 @@ def main():
         line["e2e"] = e2e
     if not args.no_cpu_baseline:
         swl, desc, _ = oracle_sample(args.workload, K)
-        osteps = 100 if swl.dim == 3 else 2000
+        osteps = 600 if swl.dim == 3 else 4000   # about 10-20 s of CPU work
         val, dt, zz, cores = time_oracle(swl, osteps)
         line["cpu_baseline"] = {"value": val, "unit": "node-steps/s", "cores": cores, "kind": "oracle",
                                 "sample": f"{desc}, {osteps} steps, {dt:.1f} s"}
