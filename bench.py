@@ -108,8 +108,8 @@ def time_oracle(wl, steps):
 
 
 def run_reference(args):
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    from paper_2309_11273_b200 import replicas
+    if replicas.rank_info()[0] != 0:   # under torchrun rank 0 alone runs and prints the reference arm
         return 0
     wl, desc, _ = oracle_sample(args.workload, args.steps)
     per_step = max(1, min(args.steps, 50 if wl.dim == 3 else 500))
@@ -147,9 +147,8 @@ def main():
     import torch.distributed as dist
     from paper_2309_11273_b200 import pd
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2309_11273_b200 import replicas
+    rank, local, world = replicas.rank_info()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
     torch.cuda.set_device(local)
@@ -193,10 +192,7 @@ def main():
     nk = min(K, 100)
     sampler.stop()
     clocks = sampler.summary(tw0, tw1)
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
+    ms = replicas.max_over_ranks(ms, device="cuda")
     stats = sim.get_stats()
     u_max = float(np.abs(sim.get_u()).max()) if rank == 0 else 0.0
     sim.destroy()
@@ -216,11 +212,8 @@ def main():
         te = time.perf_counter() - t0
         d2h = uo.nbytes + vo.nbytes + do.nbytes
         sim2.destroy()
-        tt = torch.tensor([te], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        te = float(tt.item())
-        e2e = {"value": world * n * K / te, "unit": "node-steps/s", "h2d_bytes_per_step": h2d / K,
+        te = replicas.max_over_ranks(te, device="cuda")
+        e2e = {"value": replicas.whole_job_throughput(n, K, te * 1e3, world), "unit": "node-steps/s", "h2d_bytes_per_step": h2d / K,
                "d2h_bytes_per_step": d2h / K, "seconds": te,
                "note": "pd_create from host arrays (family build included) + pd_step(K) + pd_get_u/v/damage to host"}
 
@@ -249,14 +242,14 @@ def main():
     achieved = dom[1] / dom[2] / 1e9
     step_s = ms * 1e-3 / K
     line = {
-        "metric": METRIC, "value": world * n * K / (ms * 1e-3), "unit": "node-steps/s", "n_gpus": world, "steps": K,
+        "metric": METRIC, "value": replicas.whole_job_throughput(n, K, ms, world), "unit": "node-steps/s", "n_gpus": world, "steps": K,
         "warmup": Wm, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"{args.workload}:{wl.name}", "nodes": n, "directed_bonds": z, "dim": wl.dim,
                    "fracture": bool(fracture), "horizon_over_dx": 3.015, "l2": "inputs larger than L2 (no flush needed)"
                    if 4 * z > 2 * 126e6 else "working set fits L2: HBM fraction not meaningful", "parallelism":
                    "replicas only" if world > 1 else "1 GPU", "build_seconds": t_build, "layout": lay},
-        "bond_updates_per_s": world * z * K / (ms * 1e-3),
+        "bond_updates_per_s": replicas.whole_job_throughput(z, K, ms, world),
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": {"bound": "hbm", "kernel": dom[0], "achieved": achieved, "peak": peak, "unit": "GB/s",

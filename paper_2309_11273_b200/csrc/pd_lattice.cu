@@ -66,15 +66,19 @@ __global__ void k_lat_offsets(int64_t n, PdGrid g, double h2, const double *__re
         const int x = cx + dx, y = cy + dy, z = cz + dz;
         if (x < 0 || y < 0 || z < 0 || x >= g.nc[0] || y >= g.nc[1] || z >= g.nc[2]) continue;
         if (dx == 0 && dy == 0 && dz == 0) continue;
+        const int o = ((dz + g.S[2]) * wy + (dy + g.S[1])) * wx + (dx + g.S[0]);
+        if ((bitmap[o >> 5] >> (o & 31)) & 1u) continue;   // already known to occur
+        {   // nodes sit within half a cell of their cell centre: coordinates differ by >= (|d| - 1) cell edges
+          const double lx = max(abs(dx) - 1, 0) / g.inv_c[0], ly = max(abs(dy) - 1, 0) / g.inv_c[1],
+                       lz = g.dim > 2 ? max(abs(dz) - 1, 0) / g.inv_c[2] : 0.0;
+          if (lx * lx + ly * ly + lz * lz > h2 * (1.0 + 1e-9)) continue;
+        }
         const int64_t cell = ((int64_t)z * g.nc[1] + y) * g.nc[0] + x;
         const int32_t q = cell_start[cell];
         if (cell_end[cell] <= q) continue;
         double pj[3] = {0, 0, 0};
         for (int k = 0; k < g.dim; ++k) pj[k] = coords[(int64_t)g.dim * ids[q] + g.ax[k]];
-        if (dist2_exact(g.dim, pi, pj) <= h2) {
-          const int o = ((dz + g.S[2]) * wy + (dy + g.S[1])) * wx + (dx + g.S[0]);
-          if (!((bitmap[o >> 5] >> (o & 31)) & 1u)) atomicOr(&bitmap[o >> 5], 1u << (o & 31));
-        }
+        if (dist2_exact(g.dim, pi, pj) <= h2) atomicOr(&bitmap[o >> 5], 1u << (o & 31));
       }
 }
 
