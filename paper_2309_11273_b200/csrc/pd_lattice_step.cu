@@ -131,6 +131,8 @@ namespace {
 
 template <int DIM, bool FORCE, bool FRAC> struct PolicyOf { using type = pdb::DilPolicy<DIM, FRAC, true, 4, true>; };
 template <int DIM, bool FRAC> struct PolicyOf<DIM, true, FRAC> { using type = pdb::ForcePolicy<DIM, true, 4>; };
+template <int DIM, bool FORCE, bool FRAC, int R> struct PolicyOfR { using type = pdb::DilPolicy<DIM, FRAC, true, R, true>; };
+template <int DIM, bool FRAC, int R> struct PolicyOfR<DIM, true, FRAC, R> { using type = pdb::ForcePolicy<DIM, true, R>; };
 
 // shared-memory carve-up (bytes), the same on host and device
 struct LatSmem {
@@ -420,49 +422,55 @@ __device__ __forceinline__ void ldg_ent_if(E &e, const double2 *const (&pk)[NPAI
   if (NPAIR > DIMP) ldg_if(e.g, pk[DIMP] + off, pred);
 }
 
-template <bool MASKED, bool STAGED, int NPAIR, class P>
+// R rows per lane (R = 4: one record serves up to 4 bonds; R = 2: half the registers, twice the warps)
+template <bool MASKED, bool STAGED, int NPAIR, int R, class P>
 __device__ __forceinline__ void dir_run_col(P &p, const double2 *const (&pk)[NPAIR], int base, int DX, int n,
-                                            const uint32_t (&bits)[4], const uint32_t (&nfb)[4], uint32_t (&clr)[4],
+                                            const uint32_t (&bits)[R], const uint32_t (&nfb)[R], uint32_t (&clr)[R],
                                             const int *thr) {
-  typename P::E S[4];
+  typename P::E S[R];
 #pragma unroll
-  for (int q = 0; q < 4; ++q) ldg_ent<NPAIR>(S[q], pk, base + q * DX);
+  for (int q = 0; q < R; ++q) ldg_ent<NPAIR>(S[q], pk, base + q * DX);
   uint32_t anyp = 0;
-  if (MASKED) anyp = __reduce_or_sync(FULL, bits[0] | (bits[1] << 7) | (bits[2] << 14) | (bits[3] << 21));
+  if (MASKED) {
+    uint32_t pkd = 0;
+#pragma unroll
+    for (int r = 0; r < R; ++r) pkd |= bits[r] << (7 * r);
+    anyp = __reduce_or_sync(FULL, pkd);
+  }
+  constexpr uint32_t STEPBITS = R == 4 ? 0x204081u : (R == 2 ? 0x81u : 0x1u);
   auto bond = [&](int r, const typename P::E &e, int t) {
     if (p.template bond<MASKED>(r, e, (bits[r] >> t) & 1u, (nfb[r] >> t) & 1u)) clr[r] |= 1u << t;
   };
 #pragma unroll
   for (int t = 0; t < PD_MAXSTEP; ++t) {
     if (t < n) {
-      const bool live = !MASKED || (anyp & (0x204081u << t)) != 0;   // warp-uniform
+      const bool live = !MASKED || (anyp & (STEPBITS << t)) != 0;   // warp-uniform
       if (STAGED) {
-        // differences of the 4 rows first (row 0 frees its slot for the next record), then the products
+        // differences of the R rows first (row 0 frees its slot for the next record), then the products
         // phase by phase over the rows (pd_bond.cuh, finish)
-        if (live) p.diffs(0, S[t % 4]);
-        ldg_ent_if<NPAIR>(S[t % 4], pk, base + (t + 4) * DX, (t + 1 < n) ? 1u : 0u);
+        if (live) p.diffs(0, S[t % R]);
+        ldg_ent_if<NPAIR>(S[t % R], pk, base + (t + R) * DX, (t + 1 < n) ? 1u : 0u);
         if (live) {
-          p.diffs(1, S[(t + 1) % 4]);
-          p.diffs(2, S[(t + 2) % 4]);
-          p.diffs(3, S[(t + 3) % 4]);
-          uint32_t in4 = 15u, nf4 = 0u;
+#pragma unroll
+          for (int r = 1; r < R; ++r) p.diffs(r, S[(t + r) % R]);
+          uint32_t in4 = (1u << R) - 1u, nf4 = 0u;
           if (MASKED) {
-            in4 = ((bits[0] >> t) & 1u) | (((bits[1] >> t) & 1u) << 1) | (((bits[2] >> t) & 1u) << 2) | (((bits[3] >> t) & 1u) << 3);
-            nf4 = ((nfb[0] >> t) & 1u) | (((nfb[1] >> t) & 1u) << 1) | (((nfb[2] >> t) & 1u) << 2) | (((nfb[3] >> t) & 1u) << 3);
+            in4 = 0;
+#pragma unroll
+            for (int r = 0; r < R; ++r) { in4 |= ((bits[r] >> t) & 1u) << r; nf4 |= ((nfb[r] >> t) & 1u) << r; }
           }
           const uint32_t brk = p.template finish<MASKED>(in4, nf4);
           if (MASKED && P::kFrac) {
 #pragma unroll
-            for (int r = 0; r < 4; ++r) clr[r] |= ((brk >> r) & 1u) << t;
+            for (int r = 0; r < R; ++r) clr[r] |= ((brk >> r) & 1u) << t;
           }
         }
       } else {
-        if (live) bond(0, S[t % 4], t);
-        ldg_ent_if<NPAIR>(S[t % 4], pk, base + (t + 4) * DX, (t + 1 < n) ? 1u : 0u);   // record t+4: row 3 of step t+1
+        if (live) bond(0, S[t % R], t);
+        ldg_ent_if<NPAIR>(S[t % R], pk, base + (t + R) * DX, (t + 1 < n) ? 1u : 0u);   // record t+R: last row of step t+1
         if (live) {
-          bond(1, S[(t + 1) % 4], t);
-          bond(2, S[(t + 2) % 4], t);
-          bond(3, S[(t + 3) % 4], t);
+#pragma unroll
+          for (int r = 1; r < R; ++r) bond(r, S[(t + r) % R], t);
         }
       }
       if (!MASKED && P::kFrac) p.step_end(thr[t]);
@@ -473,7 +481,7 @@ __device__ __forceinline__ void dir_run_col(P &p, const double2 *const (&pk)[NPA
 struct DirArgs {
   int DX, DY, HX, HY, HZ, PZ;
   int nxc, nyq, nyq_used;            // x chunks; rgocc stride; row groups along y that can hold nodes
-  int ncol, nw, cy, cz;              // columns; mask words; row groups (y) and levels (z) per CTA
+  int ncol, nw, cy, cz, rows;        // columns; mask words; row groups (y) and levels (z) per CTA; rows per lane
   int64_t npad;
   const double2 *nbr;
   double2 *nbw;
@@ -490,34 +498,34 @@ struct DirArgs {
   struct Col { int off; uint8_t n, word, bit0, pad; } cols[PD_LAT_MAXCOL];   // off = (dz*DY + dy0)*DX + dx (dense cells)
 };
 
-template <int DIM, bool FORCE, bool FRAC, int MAXT, int MINB, bool STAGED>
+template <int DIM, bool FORCE, bool FRAC, int MAXT, int MINB, bool STAGED, int R>
 __global__ void __launch_bounds__(MAXT, MINB) k_lat_direct(const __grid_constant__ DirArgs a) {
   extern __shared__ __align__(16) unsigned char smraw[];
   constexpr int NPAIR = FORCE ? DIM + 1 : DIM;
-  using P = typename PolicyOf<DIM, FORCE, FRAC>::type;
+  using P = typename PolicyOfR<DIM, FORCE, FRAC, R>::type;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
   // shared: column table, thresholds, per-warp mask words [nwarp][4 words][4 rows][32]
   DirArgs::Col *scol = (DirArgs::Col *)smraw;
   int *sthr = (int *)(scol + a.ncol);
-  uint32_t *smk = (uint32_t *)(sthr + (FORCE ? 0 : a.ncol * 8)) + warp * 512;
+  uint32_t *smk = (uint32_t *)(sthr + (FORCE ? 0 : a.ncol * 8)) + warp * (128 * R);
   for (int c = tid; c < a.ncol; c += blockDim.x) scol[c] = a.cols[c];
   if (!FORCE && a.thr)
     for (int c = tid; c < a.ncol * 8; c += blockDim.x) sthr[c] = a.thr[c];
   // this warp's row group: (xc, yq, z)
   const int wy = warp % a.cy, wz = warp / a.cy;
-  const int xc = blockIdx.x, yq = blockIdx.y * a.cy + wy, z = blockIdx.z * a.cz + wz;
-  const bool active = yq < a.nyq_used && z < a.PZ && a.rgocc[((int64_t)z * a.nyq + yq) * a.nxc + xc] != 0;
-  const int64_t i0 = ((int64_t)(z + a.HZ) * a.DY + (yq * 4 + a.HY)) * a.DX + (xc * 32 + lane + a.HX);   // row 0's cell
+  const int xc = blockIdx.x, yq = blockIdx.y * a.cy + wy, z = blockIdx.z * a.cz + wz;   // yq counts groups of R rows
+  const bool active = yq < a.nyq_used && z < a.PZ && a.rgocc[((int64_t)z * a.nyq + ((yq * R) >> 2)) * a.nxc + xc] != 0;
+  const int64_t i0 = ((int64_t)(z + a.HZ) * a.DY + (yq * R + a.HY)) * a.DX + (xc * 32 + lane + a.HX);   // row 0's cell
   if (active) {
 #pragma unroll
-    for (int r = 0; r < 4; ++r)
-      for (int w = 0; w < a.nw; ++w) smk[(w * 4 + r) * 32 + lane] = a.mask[(int64_t)w * a.npad + i0 + (int64_t)r * a.DX];
+    for (int r = 0; r < R; ++r)
+      for (int w = 0; w < a.nw; ++w) smk[(w * R + r) * 32 + lane] = a.mask[(int64_t)w * a.npad + i0 + (int64_t)r * a.DX];
   }
   __syncthreads();   // tables visible (the only CTA barrier)
   if (!active) return;
   P p;
 #pragma unroll
-  for (int r = 0; r < 4; ++r) {
+  for (int r = 0; r < R; ++r) {
 #pragma unroll
     for (int k = 0; k < DIM; ++k) {
       const double2 xu = a.nbr[(int64_t)k * a.npad + i0 + (int64_t)r * a.DX];
@@ -527,7 +535,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_lat_direct(const __grid_constant
   }
   if constexpr (FORCE) {
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
+    for (int r = 0; r < R; ++r) {
       const double2 g = a.nbr[(int64_t)PD_P_AUX * a.npad + i0 + (int64_t)r * a.DX];
       p.gmu_i[r] = g.x;
       p.cth_i[r] = g.y;
@@ -537,7 +545,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_lat_direct(const __grid_constant
   } else {
     p.s_c = a.s_c;
 #pragma unroll
-    for (int r = 0; r < 4; ++r) p.acc[r] = 0.0;
+    for (int r = 0; r < R; ++r) p.acc[r] = 0.0;
   }
   const double2 *pk[NPAIR];   // pair k of the warp's own row-0 cell: a record is pk[k] + (32-bit cell offset)
 #pragma unroll
@@ -547,43 +555,48 @@ __global__ void __launch_bounds__(MAXT, MINB) k_lat_direct(const __grid_constant
     const DirArgs::Col col = scol[c];
     const int n = col.n;
     const uint32_t nmask = (1u << n) - 1u;
-    uint32_t bits[4], nfb[4] = {0, 0, 0, 0}, clr[4] = {0, 0, 0, 0};
+    uint32_t bits[R], nfb[R], clr[R];
 #pragma unroll
-    for (int r = 0; r < 4; ++r) bits[r] = (smk[(col.word * 4 + r) * 32 + lane] >> col.bit0) & nmask;
-    bool slow = !__all_sync(FULL, (bits[0] & bits[1] & bits[2] & bits[3]) == nmask);
+    for (int r = 0; r < R; ++r) nfb[r] = clr[r] = 0;
+#pragma unroll
+    for (int r = 0; r < R; ++r) bits[r] = (smk[(col.word * R + r) * 32 + lane] >> col.bit0) & nmask;
+    uint32_t ball = bits[0];
+#pragma unroll
+    for (int r = 1; r < R; ++r) ball &= bits[r];
+    bool slow = !__all_sync(FULL, ball == nmask);
     const int base = col.off;
     const int *thr = sthr + 8 * c;
     if (!slow) {
       p.fast_begin();
-      dir_run_col<false, STAGED, NPAIR>(p, pk, base, a.DX, n, bits, nfb, clr, thr);
+      dir_run_col<false, STAGED, NPAIR, R>(p, pk, base, a.DX, n, bits, nfb, clr, thr);
       slow = p.fast_failed();
     }
     if (slow) {
       if (P::kFrac && a.nofail) {
 #pragma unroll
-        for (int r = 0; r < 4; ++r) nfb[r] = (a.nofail[(int64_t)col.word * a.npad + i0 + (int64_t)r * a.DX] >> col.bit0) & nmask;
+        for (int r = 0; r < R; ++r) nfb[r] = (a.nofail[(int64_t)col.word * a.npad + i0 + (int64_t)r * a.DX] >> col.bit0) & nmask;
       }
-      dir_run_col<true, STAGED, NPAIR>(p, pk, base, a.DX, n, bits, nfb, clr, thr);
+      dir_run_col<true, STAGED, NPAIR, R>(p, pk, base, a.DX, n, bits, nfb, clr, thr);
       if (P::kFrac) {
 #pragma unroll
-        for (int r = 0; r < 4; ++r)
-          if (clr[r]) { smk[(col.word * 4 + r) * 32 + lane] &= ~(clr[r] << col.bit0); dirty = true; }
+        for (int r = 0; r < R; ++r)
+          if (clr[r]) { smk[(col.word * R + r) * 32 + lane] &= ~(clr[r] << col.bit0); dirty = true; }
       }
     }
   }
   if (FRAC && __any_sync(FULL, dirty)) {   // broken bits back to HBM
     if (dirty) {
 #pragma unroll
-      for (int r = 0; r < 4; ++r)
-        for (int w = 0; w < a.nw; ++w) a.mask[(int64_t)w * a.npad + i0 + (int64_t)r * a.DX] = smk[(w * 4 + r) * 32 + lane];
+      for (int r = 0; r < R; ++r)
+        for (int w = 0; w < a.nw; ++w) a.mask[(int64_t)w * a.npad + i0 + (int64_t)r * a.DX] = smk[(w * R + r) * 32 + lane];
     }
   }
   if constexpr (!FORCE) {
-    double mi[4];
+    double mi[R];
 #pragma unroll
-    for (int r = 0; r < 4; ++r) mi[r] = a.minv[i0 + (int64_t)r * a.DX];
+    for (int r = 0; r < R; ++r) mi[r] = a.minv[i0 + (int64_t)r * a.DX];
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
+    for (int r = 0; r < R; ++r) {
       const int64_t i = i0 + (int64_t)r * a.DX;
       const double theta = a.A * mi[r] * (p.acc[r] * a.vol_uniform);   // minv = 0 for phantoms
       a.nbw[(int64_t)PD_P_AUX * a.npad + i] = make_double2(a.G * mi[r], a.c1 * theta * mi[r]);
@@ -591,16 +604,16 @@ __global__ void __launch_bounds__(MAXT, MINB) k_lat_direct(const __grid_constant
     }
   } else {
     // ---- Eq. 2.11 + boundary dofs (App. B) ----
-    double vk[4][DIM];
-    unsigned fl[4];
+    double vk[R][DIM];
+    unsigned fl[R];
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
+    for (int r = 0; r < R; ++r) {
       fl[r] = a.flags32[i0 + (int64_t)r * a.DX];
 #pragma unroll
       for (int k = 0; k < DIM; ++k) vk[r][k] = a.v[k][i0 + (int64_t)r * a.DX];
     }
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
+    for (int r = 0; r < R; ++r) {
       if (p.gmu_i[r] == 0.0) continue;   // phantom (a node has m_i > 0)
       const int64_t i = i0 + (int64_t)r * a.DX;
 #pragma unroll
@@ -835,7 +848,9 @@ DirPrepared *dir_prepare(pd_sim *s, bool force) {
   slot = pp;
   DirArgs &a = pp->a;
   a.DX = l.DX; a.DY = l.DY; a.HX = l.HX; a.HY = l.HY; a.HZ = l.HZ; a.PZ = l.PZ;
-  a.nxc = l.PX / 32; a.nyq = (l.PY + 8) / 4; a.nyq_used = l.PY / 4;
+  a.rows = env_int(force ? "PD_DIR_FRC_ROWS" : "PD_DIR_DIL_ROWS", s->dim == 2 ? 2 : 4);   // rows per lane
+  if (a.rows != 2 && !(a.rows == 1 && s->dim == 2)) a.rows = 4;
+  a.nxc = l.PX / 32; a.nyq = (l.PY + 8) / 4; a.nyq_used = l.PY / a.rows;
   a.ncol = l.ncol; a.nw = l.nw;
   a.cy = std::max(1, std::min(env_int(force ? "PD_DIR_FRC_CY" : "PD_DIR_DIL_CY", 2), 4));
   a.cz = s->dim == 3 ? std::max(1, std::min(env_int(force ? "PD_DIR_FRC_CZ" : "PD_DIR_DIL_CZ", 2), 4)) : 1;
@@ -869,7 +884,7 @@ DirPrepared *dir_prepare(pd_sim *s, bool force) {
     a.thr = l.thr_dir;
   }
   const int nwarp = a.cy * a.cz;
-  pp->smem = (size_t)l.ncol * 8 + (force ? 0 : (size_t)l.ncol * 32) + (size_t)nwarp * 2048;
+  pp->smem = (size_t)l.ncol * 8 + (force ? 0 : (size_t)l.ncol * 32) + (size_t)nwarp * 512 * a.rows;
   pp->block = dim3((unsigned)(nwarp * 32));
   pp->grid = dim3((unsigned)a.nxc, (unsigned)((a.nyq_used + a.cy - 1) / a.cy), (unsigned)((l.PZ + a.cz - 1) / a.cz));
   return pp;
@@ -888,10 +903,12 @@ int dir_launch(pd_sim *s, bool force, double *theta_out, bool frac) {
     return PD_ERR_ALLOC;
   }
   static const int staged = env_int("PD_DIR_STAGED", 2);   // bit 0: dilatation, bit 1: force (phase-ordered step, pd_bond.cuh)
-#define DIR_LAUNCH(DIM_, FORCE_, FRAC_, MINB_, ST_)                                                                      \
-  do {                                                                                                                   \
-    if (ST_) k_lat_direct<DIM_, FORCE_, FRAC_, 128, MINB_, true><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);       \
-    else k_lat_direct<DIM_, FORCE_, FRAC_, 128, MINB_, false><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);          \
+#define DIR_LAUNCH(DIM_, FORCE_, FRAC_, MINB_, ST_)                                                                        \
+  do {                                                                                                                     \
+    if (a.rows == 1 && DIM_ == 2) k_lat_direct<2, FORCE_, FRAC_, 128, 4, false, 1><<<pp->grid, pp->block, pp->smem, s->stream>>>(a); \
+    else if (a.rows == 2) k_lat_direct<DIM_, FORCE_, FRAC_, 128, (FORCE_ ? 3 : 4), false, 2><<<pp->grid, pp->block, pp->smem, s->stream>>>(a); \
+    else if (ST_) k_lat_direct<DIM_, FORCE_, FRAC_, 128, MINB_, true, 4><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);  \
+    else k_lat_direct<DIM_, FORCE_, FRAC_, 128, MINB_, false, 4><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);          \
   } while (0)
   if (force) {
     if (s->dim == 2) DIR_LAUNCH(2, true, false, 2, staged & 2); else DIR_LAUNCH(3, true, false, 2, staged & 2);

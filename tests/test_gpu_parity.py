@@ -16,6 +16,7 @@ TOL = 1e-10
 # environment switches exist for exactly this purpose (and for profiling)
 LAYOUTS = {
     "lattice_direct": ({}, 1),
+    "lattice_direct_2rows": ({"PD_DIR_DIL_ROWS": "2", "PD_DIR_FRC_ROWS": "2"}, 1),   # 2 instead of 4 rows per lane
     "lattice_march": ({"PD_LAT_KERNEL": "march"}, 2),
     "sliced_ell": ({"PD_FORCE_GENERIC": "1"}, 0),
 }
@@ -24,7 +25,7 @@ LAYOUTS = {
 @pytest.fixture(params=list(LAYOUTS))
 def layout(request, monkeypatch):
     env, code = LAYOUTS[request.param]
-    for k in ("PD_LAT_KERNEL", "PD_FORCE_GENERIC"):
+    for k in ("PD_LAT_KERNEL", "PD_FORCE_GENERIC", "PD_DIR_DIL_ROWS", "PD_DIR_FRC_ROWS"):
         monkeypatch.delenv(k, raising=False)
     for k, v in env.items():
         monkeypatch.setenv(k, v)
