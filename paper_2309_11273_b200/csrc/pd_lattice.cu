@@ -1,4 +1,4 @@
-// pd_lattice.cu -- dense LATTICE layout: builder and step kernels (rows a1-a5)
+// pd_lattice.cu -- dense LATTICE layout: the builder
 // for bodies discretised on a (jittered) lattice, which is the paper's discretisation.
 //
 // When every cell of the builder's cell grid holds at most one node, the volumes are uniform and

@@ -1,23 +1,24 @@
 // pd_lattice_step.cu -- step kernels of the dense lattice layout (pd_lattice.cu, PdLattice):
-// SURVEY.md 8(a) rows a1-a5 for (jittered) lattice bodies.
+// SURVEY.md 8(a) rows a1-a5 for (jittered) lattice bodies.  Two families, same layout, same per-bond
+// arithmetic (pd_bond.cuh, shared with pd_step.cu):
 //
-// "2.5-D" marching: a CTA owns a COLUMN of cells, 32 (x, the lane axis) by TY (y), and marches
-// through LZ levels of z.  Shared memory holds a RING of 2 HZ + 2 z-PLANES of neighbour records,
-// each plane = the column's 32 x TY cells plus a halo of the stencil radius in x and y.  While
-// level z is computed from the planes z - HZ .. z + HZ, plane z + HZ + 1 (and the mask words and
-// update operands of level z + 1) arrive through 16-byte asynchronous copies (cp.async): every
-// HBM/L2 access of the step is a coalesced row copy one level ahead of its use, each record is
-// fetched about (TY + 2 HY)(32 + 2 HX) / (32 TY) = 2-3 times per pass instead of once per bond, and
-// the ~120 gathers per node are shared-memory reads.
+// (1) DIRECT kernels `k_lat_direct` -- the default.  One warp owns a ROW GROUP (32 lanes x R rows
+//     adjacent in y, R = 4 in 3-D) at one level and walks all stencil COLUMNS (dx, dy0..dy0+n-1, dz)
+//     with an R-record register window sliding along y: in step t row r pairs with record t + r, one
+//     gathered record serves up to R bonds, the R bonds of a step are independent FP64 chains in one
+//     basic block.  Records are read straight from the dense pair arrays by arithmetic addressing
+//     (16-byte loads, 512 contiguous bytes per pair and warp, shared between warps through L1); there
+//     is no shared-memory staging and no CTA barrier.  A column whose R n bonds are intact on all 32
+//     lanes runs without a single mask test (FAST); otherwise the MASKED variant predicates the
+//     accumulation and, in the dilatation pass, clears the bits of the bonds that break (Eq. 1.30).
 //
-// Inside a level a warp owns a ROW GROUP (32 lanes x 4 rows adjacent in y).  The stencil columns
-// (dx, dy0 .. dy0 + n - 1, dz) are walked with a 4-record register window sliding along y: in step
-// t row r pairs with record t + r, one shared-memory record serves 4 bonds, the 4 bonds of a step
-// are independent FP64 chains in one basic block.  NSPLIT warps share a row group by splitting the
-// stencil columns between them; their partial sums are added through shared memory.  A column
-// whose 4 n bonds are intact on all 32 lanes runs without a single mask test (FAST); otherwise the
-// MASKED variant predicates the accumulation and, in the dilatation pass, clears the bits of the
-// bonds that break (Eq. 1.30).  The per-bond arithmetic is pd_bond.cuh, shared with pd_step.cu.
+// (2) MARCHING kernels `k_lat_march` (PD_LAT_KERNEL=march; kept as the measured alternative, see
+//     profiles/r01b_design_history.md).  "2.5-D" marching: a CTA owns a column of cells, 32 (x) by
+//     TY (y), and marches through LZ levels of z.  Shared memory holds a RING of 2 HZ + 2 z-PLANES of
+//     neighbour records (the column's cells plus a halo of the stencil radius in x and y).  While
+//     level z is computed from the planes z - HZ .. z + HZ, plane z + HZ + 1 and the mask words and
+//     update operands of level z + 1 arrive through asynchronous copies (cp.async); NSPLIT warps
+//     share a row group by splitting the stencil columns, their partial sums meet in shared memory.
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
