@@ -1,6 +1,7 @@
 // pd_api.cu -- the C-ABI entry points of include/pd.h: argument checks, staging of caller data,
 // the step loop, and read-back in user node order.  No numerics of the method live here except
 // the three mode constants A, K, G (Eqs. 1.8, 1.15, 1.16).
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -16,31 +17,50 @@ inline unsigned nblk(int64_t n) { return (unsigned)((n + TPB - 1) / TPB); }
 // user AoS (dim*n) -> final order; dst is either the u half of the position pairs of a neighbour-record
 // buffer (nb != NULL) or SoA arrays
 struct Ax { int a[3]; };
+// where a vector field lives: the u half of the position pairs of a neighbour-record buffer (nb), the
+// {u_0, u_1} / u_2 arrays of the uniform lattice layout (uxy, uz), or SoA arrays (d)
+struct FieldView {
+  double2 *nb; bool lattice;
+  double2 *uxy; double *uz;
+  double *d[3];
+};
+__device__ __forceinline__ double &field_ref(const FieldView &f, int64_t npad, int64_t i, int k) {
+  if (f.nb) return f.nb[pd_pair_index(f.lattice, npad, i, k)].y;
+  if (f.uxy) return k == 0 ? f.uxy[i].x : (k == 1 ? f.uxy[i].y : f.uz[i]);
+  return f.d[k][i];
+}
 __global__ void k_scatter_field(int64_t npad, int dim, Ax ax, const int32_t *__restrict__ perm, const double *__restrict__ src,
-                                const uint8_t *__restrict__ flags, bool clamp_zero, double2 *nb, bool lattice, double *d0,
-                                double *d1, double *d2) {
+                                const uint8_t *__restrict__ flags, bool clamp_zero, FieldView f) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= npad) return;
-  double *d[3] = {d0, d1, d2};
   int32_t uidx = perm[i];
   unsigned fl = flags[i];
   for (int k = 0; k < dim; ++k) {
     double val = (src && uidx >= 0) ? src[(int64_t)dim * uidx + ax.a[k]] : 0.0;
     if (clamp_zero && (fl & (1u << k))) val = 0.0;
-    if (nb) nb[pd_pair_index(lattice, npad, i, k)].y = val; else d[k][i] = val;
+    field_ref(f, npad, i, k) = val;
   }
 }
 
 // final order -> user AoS; source is the u half of a neighbour-record buffer or SoA arrays
-__global__ void k_gather_field(int64_t npad, int dim, Ax ax, const int32_t *__restrict__ perm, const double2 *__restrict__ nb, bool lattice,
-                               const double *__restrict__ s0, const double *__restrict__ s1,
-                               const double *__restrict__ s2, double *dst) {
+__global__ void k_gather_field(int64_t npad, int dim, Ax ax, const int32_t *__restrict__ perm, FieldView f, double *dst) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= npad) return;
-  const double *s[3] = {s0, s1, s2};
   int32_t uidx = perm[i];
   if (uidx < 0) return;
-  for (int k = 0; k < dim; ++k) dst[(int64_t)dim * uidx + ax.a[k]] = nb ? nb[pd_pair_index(lattice, npad, i, k)].y : s[k][i];
+  for (int k = 0; k < dim; ++k) dst[(int64_t)dim * uidx + ax.a[k]] = field_ref(f, npad, i, k);
+}
+
+FieldView view_u(pd_sim *s, int buf) {
+  FieldView f{};
+  if (s->lat.on && s->lat.uniform) { f.uxy = s->lat.uxy[buf]; f.uz = s->lat.uz[buf]; }
+  else { f.nb = s->nb[buf]; f.lattice = s->lat.on; }
+  return f;
+}
+FieldView view_soa(double *const *d) {
+  FieldView f{};
+  for (int k = 0; k < 3; ++k) f.d[k] = d[k];
+  return f;
 }
 
 // scalar per node
@@ -76,11 +96,13 @@ int stage(pd_sim *s, const void *src, size_t bytes, void **out) {
   return PD_OK;
 }
 
-void flush_break(pd_sim *s) {  // deferred step 5: decide rho^{n} from u^{n} before anything reads it
+int flush_break(pd_sim *s) {  // deferred step 5: decide rho^{n} from u^{n} before anything reads it
   if (s->fracture && s->break_pending) {
-    pdi::launch_dilatation(s, nullptr, true);
+    const int rc = pdi::launch_dilatation(s, nullptr, true);
+    if (rc) return rc;
     s->break_pending = false;
   }
+  return PD_OK;
 }
 
 int copy_out(pd_sim *s, void *dst, const void *src_dev, size_t bytes) {
@@ -93,8 +115,8 @@ int get_field(pd_sim *s, double *dst, bool velocity) {
   if (!s || !dst) { pdi::set_error("null argument"); return PD_ERR_ARG; }
   DevTmp tmp(s, sizeof(double) * s->dim * s->n);
   if (!tmp.p) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
-  k_gather_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, velocity ? nullptr : s->nb[s->cur], s->lat.on,
-                                                       s->v[0], s->v[1], s->v[2], (double *)tmp.p);
+  k_gather_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm,
+                                                       velocity ? view_soa(s->v) : view_u(s, s->cur), (double *)tmp.p);
   PD_CUDA(cudaGetLastError());
   return copy_out(s, dst, tmp.p, sizeof(double) * s->dim * s->n);
 }
@@ -137,7 +159,10 @@ void dev_free_all(pd_sim *s) {
 extern "C" {
 
 const char *pd_last_error(void) { return g_err.c_str(); }
-const char *pd_version(void) { return "pd-b200 0.3 (sm_100a, FP64, windowed SELL-32x4, warp per 4-row group)"; }
+const char *pd_version(void) {
+  return "pd-b200 0.4 (sm_100a, FP64; layouts: uniform lattice [constant bond geometry per stencil offset], dense lattice, "
+         "windowed sliced ELL; warp per 32 x R row group)";
+}
 
 int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volumes, double horizon,
               const pd_material *mat, const pd_boundary *bc, const pd_runtime *rt) {
@@ -208,30 +233,92 @@ int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volum
     ok = s->stats_dev != nullptr;
   }
   if (!ok) { pdi::set_error("device allocation failed for the state arrays"); return fail(PD_ERR_ALLOC); }
-  k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, (const double *)d_u0, s->flags, true,
-                                                         s->nb[0], s->lat.on, nullptr, nullptr, nullptr);
-  k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, (const double *)d_v0, s->flags, true,
-                                                         nullptr, false, s->v[0], s->v[1], s->v[2]);
-  k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->perm, (const double *)d_val, s->flags, false,
-                                                         nullptr, false, s->bval[0], s->bval[1], s->bval[2]);
+  const Ax axv{{s->ax[0], s->ax[1], s->ax[2]}};
+  k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, axv, s->perm, (const double *)d_u0, s->flags, true, view_u(s, 0));
+  k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, axv, s->perm, (const double *)d_v0, s->flags, true, view_soa(s->v));
+  k_scatter_field<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, axv, s->perm, (const double *)d_val, s->flags, false,
+                                                         view_soa(s->bval));
   cudaError_t e = cudaGetLastError();
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
   if (e != cudaSuccess) return fail(pdi::cuda_fail(e, "pd_create state initialisation"));
   for (void *p : {d_coords, d_vol, d_flags, d_precut, d_u0, d_v0, d_val}) pdi::dev_free(s, p);
   s->cur = 0; s->step = 0; s->break_pending = false;  // u^0 is not break-checked (reading C-5)
+  if (const char *env = getenv("PD_GRAPH")) s->use_graph = atoi(env) != 0;
+  if (const char *env = getenv("PD_GRAPH_STEPS")) s->graph_len = std::max(2, std::min(atoi(env) & ~1, 256));
   *out = s;
   return PD_OK;
 }
 
+// one explicit step by plain launches: rows a1, a2 (+ deferred a5), then a1, a3, a4
+static int step_once(pd_sim *s) {
+  int rc = pdi::launch_dilatation(s, nullptr, s->break_pending);
+  if (rc) return rc;
+  if ((rc = pdi::launch_force_update(s))) return rc;
+  s->cur ^= 1;
+  s->step += 1;
+  s->break_pending = s->fracture;
+  s->launches += 2;
+  return PD_OK;
+}
+
+// The step loop without per-step host work: 2 g steps (g = 1 or PD_GRAPH_STEPS / 2) are captured once into a CUDA
+// graph and replayed.  A graph bakes its kernel arguments, so it is only used in the STEADY state -- buffer parity
+// cur = 0 at its start, the deferred break test pending (or no fracture), the load ramp g(t) finished -- and every
+// other step takes plain launches.  Capture runs on a private stream (the caller's may be the legacy default
+// stream, which cannot be captured); replay is enqueued on the caller's stream.
+static bool graph_steady(const pd_sim *s) {
+  return s->cur == 0 && s->break_pending == s->fracture &&
+         (s->ramp_time <= 0.0 || (double)s->step * s->dt >= s->ramp_time);
+}
+static int graph_build(pd_sim *s, int which, int nsteps) {
+  if (!s->cap_stream && cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+    cudaGetLastError();
+    return PD_ERR_CUDA;
+  }
+  const cudaStream_t user = s->stream;
+  const int cur0 = s->cur;
+  const int64_t step0 = s->step, launches0 = s->launches;
+  s->stream = s->cap_stream;
+  cudaGraph_t g = nullptr;
+  int rc = PD_OK;
+  if (cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) rc = PD_ERR_CUDA;
+  for (int it = 0; it < nsteps && rc == PD_OK; ++it) rc = step_once(s);
+  if (cudaStreamEndCapture(s->cap_stream, &g) != cudaSuccess) rc = rc ? rc : PD_ERR_CUDA;
+  s->stream = user;
+  s->cur = cur0; s->step = step0; s->launches = launches0;   // nothing ran
+  if (rc == PD_OK && cudaGraphInstantiate(&s->graph[which], g, 0) != cudaSuccess) rc = PD_ERR_CUDA;
+  if (g) cudaGraphDestroy(g);
+  if (rc != PD_OK) { cudaGetLastError(); s->graph[which] = nullptr; }
+  else s->graph_steps[which] = nsteps;
+  return rc;
+}
+
 int pd_step(pd_sim *s, int64_t nsteps) {
   if (!s || nsteps < 0) { pdi::set_error("bad argument"); return PD_ERR_ARG; }
-  for (int64_t it = 0; it < nsteps; ++it) {
-    pdi::launch_dilatation(s, nullptr, s->break_pending);  // steps (1),(2) + deferred (5)
-    pdi::launch_force_update(s);                                     // steps (1),(3),(4)
-    s->cur ^= 1;
-    s->step += 1;
-    s->break_pending = s->fracture;
-    s->launches += 2;
+  int64_t left = nsteps;
+  while (left > 0) {
+    if (s->use_graph && left >= 2 && graph_steady(s)) {
+      // which graph: the long one when enough steps are left
+      const int big = s->graph_len;
+      const int which = (left >= big && big > 2) ? 1 : 0;
+      const int len = which ? big : 2;
+      if (!s->graph[which] && !s->graph_failed) {
+        if (s->step < 4) {   // the first steps run by plain launches (they also prepare the launch arguments)
+          if (int rc = step_once(s)) return rc;
+          --left;
+          continue;
+        }
+        if (graph_build(s, which, len) != PD_OK) s->graph_failed = true;
+      }
+      if (s->graph[which]) {
+        PD_CUDA(cudaGraphLaunch(s->graph[which], s->stream));
+        s->step += len; s->launches += 2 * len;   // cur is back at 0 after an even number of steps
+        left -= len;
+        continue;
+      }
+    }
+    if (int rc = step_once(s)) return rc;
+    --left;
   }
   PD_CUDA(cudaGetLastError());
   return PD_OK;
@@ -245,9 +332,9 @@ int pd_step_timed(pd_sim *s, int64_t nsteps, double ms[2]) {
   int rc = PD_OK;
   for (int64_t it = 0; it < nsteps && rc == PD_OK; ++it) {
     cudaEventRecord(ev[0], s->stream);
-    pdi::launch_dilatation(s, nullptr, s->break_pending);
+    if ((rc = pdi::launch_dilatation(s, nullptr, s->break_pending))) break;
     cudaEventRecord(ev[1], s->stream);
-    pdi::launch_force_update(s);
+    if ((rc = pdi::launch_force_update(s))) break;
     cudaEventRecord(ev[2], s->stream);
     s->cur ^= 1; s->step += 1; s->break_pending = s->fracture; s->launches += 2;
     cudaError_t e = cudaEventSynchronize(ev[2]);
@@ -266,8 +353,8 @@ int pd_get_v(pd_sim *s, double *dst) { return s ? get_field(s, dst, true) : PD_E
 
 int pd_get_damage(pd_sim *s, double *dst) {
   if (!s || !dst) { pdi::set_error("null argument"); return PD_ERR_ARG; }
-  flush_break(s);
-  pdi::launch_damage(s);
+  if (int rc = flush_break(s)) return rc;
+  if (int rc = pdi::launch_damage(s)) return rc;
   DevTmp tmp(s, sizeof(double) * s->n);
   if (!tmp.p) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
   k_gather_scalar<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->perm, s->phi, (double *)tmp.p);
@@ -277,8 +364,8 @@ int pd_get_damage(pd_sim *s, double *dst) {
 
 int pd_get_stats(pd_sim *s, int64_t *nbonds, int64_t *nbroken, double *max_damage, int64_t *n_ge_half, int64_t *step) {
   if (!s) { pdi::set_error("null argument"); return PD_ERR_ARG; }
-  flush_break(s);
-  pdi::launch_damage(s);
+  if (int rc = flush_break(s)) return rc;
+  if (int rc = pdi::launch_damage(s)) return rc;
   unsigned long long h[3];
   PD_CUDA(cudaMemcpyAsync(h, s->stats_dev, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
   PD_CUDA(cudaStreamSynchronize(s->stream));
@@ -300,8 +387,8 @@ int pd_get_node_fields(pd_sim *s, double *m, double *theta) {
     if (rc) return rc;
   }
   if (theta) {
-    flush_break(s);
-    pdi::launch_dilatation(s, (double *)th.p, false);
+    if (int rc = flush_break(s)) return rc;
+    if (int rc = pdi::launch_dilatation(s, (double *)th.p, false)) return rc;
     k_gather_scalar<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, s->perm, (const double *)th.p, (double *)tmp.p);
     PD_CUDA(cudaGetLastError());
     int rc = copy_out(s, theta, tmp.p, sizeof(double) * s->n);
@@ -312,7 +399,7 @@ int pd_get_node_fields(pd_sim *s, double *m, double *theta) {
 
 int pd_get_bond_mask(pd_sim *s, int64_t *rowptr, int32_t *col, uint8_t *intact) {
   if (!s || !rowptr || ((col == nullptr) != (intact == nullptr))) { pdi::set_error("bad argument"); return PD_ERR_ARG; }
-  flush_break(s);
+  if (int rc = flush_break(s)) return rc;
   DevTmp rp(s, sizeof(long long) * (s->n + 1)), c(s, col ? sizeof(int32_t) * s->Z : 1), it(s, col ? (size_t)s->Z : 1);
   if (!rp.p || !c.p || !it.p) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
   int rc = pdi::export_bond_mask(s, (long long *)rp.p, col ? (int32_t *)c.p : nullptr, col ? (uint8_t *)it.p : nullptr);
@@ -329,12 +416,15 @@ int pd_get_layout(pd_sim *s, int64_t counts[8]) {
   if (!s || !counts) { pdi::set_error("null argument"); return PD_ERR_ARG; }
   counts[0] = s->n; counts[1] = s->npad; counts[2] = s->Z; counts[3] = s->nentries * 32;
   counts[4] = s->launches; counts[5] = (int64_t)s->bytes_held; counts[6] = s->uniform_v ? 1 : 0;
-  counts[7] = s->lat.on ? 1 + s->lat.kernel : 0;
+  counts[7] = s->lat.on ? (s->lat.uniform ? 2 : 1) : 0;
   return PD_OK;
 }
 
 int pd_destroy(pd_sim *s) {
   if (!s) return PD_OK;
+  cudaStreamSynchronize(s->stream);
+  for (auto &g : s->graph) if (g) cudaGraphExecDestroy(g);
+  if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
   pdi::lat_free_cache(s);
   pdi::dev_free_all(s);
   delete s;

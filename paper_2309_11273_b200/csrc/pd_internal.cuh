@@ -110,7 +110,16 @@ struct PdGrid {
 };
 struct PdLattice {
   bool on = false;
-  int kernel = 0;                  // 0: direct kernels (default), 1: shared-memory marching kernels (PD_LAT_KERNEL=march)
+  // UNIFORM lattice (pd_lattice_uniform.cu): every bond of a stencil offset o has the same xi = (o_k h_k) up to
+  // the rounding of the coordinates, so the bond geometry is a per-offset constant and the step kernels
+  // gather displacements only:  uxy[b] = {u_0, u_1}, uz[b] = u_2 (3-D), aux = {G/m, cth}; nb[] is released.
+  bool uniform = false;
+  double h[3] = {0, 0, 0};         // lattice spacing per internal axis
+  double2 *uxy[2] = {nullptr, nullptr};
+  double *uz[2] = {nullptr, nullptr};
+  double2 *aux = nullptr;
+  double *ctab[2] = {nullptr, nullptr};   // device: per stencil bit, the constants of the dilatation / force pass
+  int wbeg[5] = {0, 0, 0, 0, 0};   // columns whose bits lie in mask word w: wbeg[w] .. wbeg[w + 1] - 1
   int DX = 0, DY = 0, DZ = 0;      // dense dims incl. margins
   int HX = 0, HY = 0, HZ = 0;      // margins = stencil radius per axis
   int PX = 0, PY = 0, PZ = 0;      // padded cell counts (PX multiple of 32, PY of 4)
@@ -123,8 +132,9 @@ struct PdLattice {
   int32_t *off2bit = nullptr;      // [(2S2+1)(2S1+1)(2S0+1)] offset -> bit index or -1
   double r2lb[128];                // per stencil bit: min over all bonds of ||xi||^2 exactly as the step kernels
                                    // compute it (break-test filter: dot < s_c * r2lb  =>  the bond cannot break)
-  void *cache[4] = {nullptr, nullptr, nullptr, nullptr};   // host: prepared launch arguments of the step kernels (pd_lattice_step.cu)
-  int32_t *thr_dev = nullptr, *thr_dir = nullptr;   // device: per (column, step) filter thresholds of the dilatation kernels
+  void *cache[4] = {nullptr, nullptr, nullptr, nullptr};   // host: prepared launch arguments of the step kernels
+                                   // ([0], [1]: pd_lattice_uniform.cu; [2], [3]: pd_lattice_step.cu)
+  int32_t *thr_dir = nullptr;      // device: per (column, step) filter thresholds of the dilatation kernel (pd_lattice_step.cu)
   int S[3] = {0, 0, 0};
 };
 
@@ -162,6 +172,12 @@ struct pd_sim {
   int64_t step = 0;       // n
   int64_t launches = 0;   // kernels launched by pd_step
   bool break_pending = false;  // u^n has not been break-checked yet (deferred step 5)
+  // CUDA graphs of the step loop (pd_api.cu): [0] = 2 steps, [1] = graph_len steps
+  bool use_graph = true, graph_failed = false;
+  int graph_len = 32;
+  int graph_steps[2] = {0, 0};
+  cudaGraphExec_t graph[2] = {nullptr, nullptr};
+  cudaStream_t cap_stream = nullptr;
   unsigned long long *stats_dev = nullptr;  // [0]=broken directed, [1]=max phi bits, [2]=#phi>=.5
 };
 
@@ -185,6 +201,10 @@ int lat_launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
 int lat_launch_force_update(pd_sim *s);
 int lat_launch_damage(pd_sim *s);
 void lat_free_cache(pd_sim *s);
+// pd_lattice_uniform.cu
+int ulat_launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
+int ulat_launch_force_update(pd_sim *s);
+void ulat_free_cache(pd_sim *s);
 // pd_step.cu
 int launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
 int launch_force_update(pd_sim *s);

@@ -13,6 +13,7 @@
 #include <cub/iterator/transform_input_iterator.cuh>
 
 #include <algorithm>
+#include <cmath>
 #include <cstdlib>
 #include <cstring>
 #include <vector>
@@ -32,6 +33,19 @@ __device__ __forceinline__ double dist2_exact(int dim, const double *a, const do
     s = __dadd_rn(s, __dmul_rn(d, d));
   }
   return s;
+}
+
+// double -> unsigned integer with the same order (and back)
+__host__ __device__ __forceinline__ unsigned long long enc_ordered(double d) {
+  unsigned long long b;
+  memcpy(&b, &d, 8);
+  return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+inline double dec_ordered(unsigned long long e) {
+  const unsigned long long b = (e >> 63) ? (e & 0x7fffffffffffffffull) : ~e;
+  double d;
+  memcpy(&d, &b, 8);
+  return d;
 }
 
 struct LatDims {
@@ -116,7 +130,7 @@ __global__ void k_lat_place(int64_t n, PdGrid g, LatDims L, const double *__rest
 __global__ void k_lat_masks(LatDims L, int dim, int nbits, double h2, double G, const int4 *__restrict__ offs,
                             const int32_t *__restrict__ perm, double2 *nb0, double2 *nb1,
                             const double *__restrict__ vol, double *mF, double *minvF, double *fvolF, int32_t *rowlen,
-                            uint32_t *member, unsigned long long *r2lb) {
+                            uint32_t *member, unsigned long long *r2lb, unsigned long long *xirange) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= L.npad || perm[i] < 0) return;
   double pi[3] = {0, 0, 0};
@@ -141,6 +155,13 @@ __global__ void k_lat_masks(LatDims L, int dim, int nbits, double h2, double G, 
         for (int k = 1; k < dim; ++k) rk = fma(xi[k], xi[k], rk);
         const unsigned long long bitsr = (unsigned long long)__double_as_longlong(rk);   // rk > 0: bit order = value order
         if (bitsr < r2lb[b]) atomicMin(&r2lb[b], bitsr);
+        // range of every component of xi over the bonds of this stencil offset (uniform-lattice test)
+        for (int k = 0; k < dim; ++k) {
+          const unsigned long long e = enc_ordered(xi[k]);
+          unsigned long long *mm = xirange + (b * 3 + k) * 2;
+          if (e < mm[0]) atomicMin(&mm[0], e);
+          if (e > mm[1]) atomicMax(&mm[1], e);
+        }
       }
       const double vj = vol[j];
       m = fma(r2, vj, m);
@@ -156,6 +177,12 @@ __global__ void k_lat_masks(LatDims L, int dim, int nbits, double h2, double G, 
   const double gmu = m > 0.0 ? G / m : 0.0;
   nb0[(int64_t)PD_P_AUX * L.npad + i].x = gmu;
   nb1[(int64_t)PD_P_AUX * L.npad + i].x = gmu;
+}
+
+// uniform lattice: the static half of the {G/m, cth} pairs
+__global__ void k_ulat_aux(int64_t npad, double G, const double *__restrict__ minv, double2 *aux) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < npad) aux[i] = make_double2(G * minv[i], 0.0);
 }
 
 __global__ void k_lat_checks(int64_t npad, const int32_t *__restrict__ perm, const int32_t *__restrict__ rowlen,
@@ -267,8 +294,6 @@ int build_lattice(pd_sim *s, const PdGrid &g, const double *coords, const double
   l.on = false;
   if (!s->uniform_v) return 0;
   if (const char *env = getenv("PD_FORCE_GENERIC")) { if (atoi(env)) return 0; }
-  l.kernel = 0;
-  if (const char *env = getenv("PD_LAT_KERNEL")) { if (!strcmp(env, "march")) l.kernel = 1; }
   const double ncell = (double)g.nc[0] * g.nc[1] * g.nc[2];
   if ((double)n < 0.2 * ncell) return 0;                      // too sparse for a dense array
   std::vector<void *> scratch;
@@ -390,8 +415,18 @@ int build_lattice(pd_sim *s, const PdGrid &g, const double *coords, const double
   unsigned long long *r2lb_d = (unsigned long long *)salloc(sizeof(unsigned long long) * 128);
   if (!r2lb_d) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
   PD_CUDA(cudaMemsetAsync(r2lb_d, 0xff, sizeof(unsigned long long) * 128, st));
+  unsigned long long *xir_d = (unsigned long long *)salloc(sizeof(unsigned long long) * 128 * 6);
+  if (!xir_d) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
+  {
+    std::vector<unsigned long long> init(128 * 6);
+    for (int q = 0; q < 128 * 3; ++q) { init[2 * q] = ~0ull; init[2 * q + 1] = 0ull; }
+    PD_CUDA(cudaMemcpyAsync(xir_d, init.data(), sizeof(unsigned long long) * 128 * 6, cudaMemcpyHostToDevice, st));
+    PD_CUDA(cudaStreamSynchronize(st));
+  }
   k_lat_masks<<<nblk(s->npad), TPB, 0, st>>>(L, dim, l.nbits, h2, s->G, offs, s->perm, s->nb[0], s->nb[1], s->vol, s->m,
-                                             s->minv, s->fvol, s->rowlen, l.member, r2lb_d);
+                                             s->minv, s->fvol, s->rowlen, l.member, r2lb_d, xir_d);
+  std::vector<unsigned long long> xir(128 * 6);
+  PD_CUDA(cudaMemcpyAsync(xir.data(), xir_d, sizeof(unsigned long long) * 128 * 6, cudaMemcpyDeviceToHost, st));
   {
     unsigned long long hb2[128];
     PD_CUDA(cudaMemcpyAsync(hb2, r2lb_d, sizeof(hb2), cudaMemcpyDeviceToHost, st));
@@ -446,6 +481,66 @@ int build_lattice(pd_sim *s, const PdGrid &g, const double *coords, const double
   }
   PD_CUDA(cudaGetLastError());
   PD_CUDA(cudaStreamSynchronize(st));
+
+  // ---- uniform lattice?  Every bond of a stencil offset o has xi = (o_k h_k) to within the rounding of the
+  //      coordinates (8 ulp of the largest coordinate per axis): the bond geometry becomes a per-offset constant
+  //      and the step kernels of pd_lattice_uniform.cu gather displacements only.  h_k = midpoint of the range
+  //      of xi_k over the bonds of the unit offset e_k (antisymmetric by construction: xi_ji = -xi_ij exactly).
+  for (int w = 0; w <= 4; ++w) {
+    int c = 0;
+    while (c < l.ncol && l.cols[c].word < w) ++c;
+    l.wbeg[w] = c;
+  }
+  l.uniform = false;
+  bool want_uniform = true;
+  if (const char *env = getenv("PD_LAT_UNIFORM")) want_uniform = atoi(env) != 0;
+  if (want_uniform) {
+    bool ok = true;
+    double h[3] = {0, 0, 0}, tol[3] = {0, 0, 0};
+    auto range = [&](int b, int k, double &lo, double &hi) {
+      const unsigned long long e0 = xir[(size_t)(b * 3 + k) * 2], e1 = xir[(size_t)(b * 3 + k) * 2 + 1];
+      if (e0 == ~0ull) return false;   // no bond with this offset
+      lo = dec_ordered(e0); hi = dec_ordered(e1);
+      return true;
+    };
+    for (int k = 0; k < dim && ok; ++k) {
+      const int e[3] = {k == 0, k == 1, k == 2};
+      const int b = has(e[0], e[1], e[2]) ? off2bit[((e[2] + g.S[2]) * wy + (e[1] + g.S[1])) * wx + (e[0] + g.S[0])] : -1;
+      double lo = 0, hi = 0;
+      if (b < 0 || !range(b, k, lo, hi) || !(lo > 0.0)) { ok = false; break; }
+      h[k] = 0.5 * (lo + hi);
+      const double cmax = std::max(std::fabs(g.lo[k]), std::fabs(g.lo[k] + (g.nc[k] - 1) / g.inv_c[k])) + h[k];
+      tol[k] = 8.0 * 2.220446049250313e-16 * cmax;
+    }
+    for (int c = 0; c < l.ncol && ok; ++c)
+      for (int t = 0; t < l.cols[c].n && ok; ++t) {
+        const int b = l.cols[c].word * 32 + l.cols[c].bit0 + t;
+        const int o[3] = {l.cols[c].dx, l.cols[c].dy0 + t, l.cols[c].dz};
+        for (int k = 0; k < dim; ++k) {
+          double lo = 0, hi = 0;
+          if (!range(b, k, lo, hi)) continue;
+          const double nominal = (double)o[k] * h[k];
+          if (std::fabs(lo - nominal) > tol[k] || std::fabs(hi - nominal) > tol[k]) ok = false;
+        }
+      }
+    if (ok) {
+      for (int k = 0; k < 3; ++k) l.h[k] = h[k];
+      for (int q = 0; q < 2; ++q) {
+        LAT_ALLOC(l.uxy[q], double2, s->npad);
+        PD_CUDA(cudaMemsetAsync(l.uxy[q], 0, sizeof(double2) * s->npad, st));
+        if (dim == 3) {
+          LAT_ALLOC(l.uz[q], double, s->npad);
+          PD_CUDA(cudaMemsetAsync(l.uz[q], 0, sizeof(double) * s->npad, st));
+        }
+      }
+      LAT_ALLOC(l.aux, double2, s->npad);
+      k_ulat_aux<<<nblk(s->npad), TPB, 0, st>>>(s->npad, s->G, s->minv, l.aux);
+      PD_CUDA(cudaGetLastError());
+      PD_CUDA(cudaStreamSynchronize(st));
+      for (int q = 0; q < 2; ++q) { dev_free(s, s->nb[q]); s->nb[q] = nullptr; }   // positions are not needed any more
+      l.uniform = true;
+    }
+  }
   return 1;
 }
 

@@ -91,12 +91,15 @@ class _TorchRuntime:
         self.torch = torch
         self.device = device
         self.live = {}
+        self.fail_allocs = False   # fault injection for the tests: every allocation fails (-> PD_ERR_ALLOC)
         self._alloc = _ALLOC_T(self._do_alloc)
         self._free = _FREE_T(self._do_free)
         self.struct = PdRuntime(self._alloc, self._free, None,
                                 C.c_void_p(torch.cuda.current_stream(device).cuda_stream))
 
     def _do_alloc(self, nbytes, _ctx):
+        if self.fail_allocs:
+            return None
         try:
             t = self.torch.empty(max(int(nbytes), 1), dtype=self.torch.uint8, device=self.device)
         except Exception:  # out of memory -> NULL -> PD_ERR_ALLOC

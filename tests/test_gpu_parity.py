@@ -12,24 +12,38 @@ pytestmark = pytest.mark.gpu
 
 TOL = 1e-10
 
-# the three code paths of the library: the layout is chosen inside pd_create; the
-# environment switches exist for exactly this purpose (and for profiling)
+# the code paths of the library: the layout is chosen inside pd_create; the environment
+# switches exist for exactly this purpose (and for profiling).  Layout codes (pd_get_layout): 2 = uniform
+# lattice (constant bond geometry per stencil offset; the default on the unjittered grids of configs 1, 2, 3, 5),
+# 1 = dense lattice with per-bond geometry (jittered config 4; PD_LAT_UNIFORM=0 forces it), 0 = sliced ELL.
 LAYOUTS = {
-    "lattice_direct": ({}, 1),
-    "lattice_direct_2rows": ({"PD_DIR_DIL_ROWS": "2", "PD_DIR_FRC_ROWS": "2"}, 1),   # 2 instead of 4 rows per lane
-    "lattice_march": ({"PD_LAT_KERNEL": "march"}, 2),
+    "default": ({}, None),
+    # rows per lane swapped (2 in 3-D, 4 in 2-D), one prefetched record in the window, plain launches instead of graphs
+    "uniform_alt": ({"PD_ULAT_DIL_ROWS": "-1", "PD_ULAT_FRC_ROWS": "-1", "PD_ULAT_DIL_PF": "1", "PD_ULAT_FRC_PF": "1",
+                     "PD_GRAPH": "0"}, None),
+    "lattice_general": ({"PD_LAT_UNIFORM": "0"}, 1),
+    "lattice_general_2rows": ({"PD_LAT_UNIFORM": "0", "PD_DIR_DIL_ROWS": "2", "PD_DIR_FRC_ROWS": "2"}, 1),
     "sliced_ell": ({"PD_FORCE_GENERIC": "1"}, 0),
 }
+_ENV_KEYS = ("PD_LAT_UNIFORM", "PD_FORCE_GENERIC", "PD_DIR_DIL_ROWS", "PD_DIR_FRC_ROWS", "PD_ULAT_DIL_ROWS",
+             "PD_ULAT_FRC_ROWS", "PD_ULAT_DIL_PF", "PD_ULAT_FRC_PF", "PD_GRAPH")
 
 
 @pytest.fixture(params=list(LAYOUTS))
 def layout(request, monkeypatch):
     env, code = LAYOUTS[request.param]
-    for k in ("PD_LAT_KERNEL", "PD_FORCE_GENERIC", "PD_DIR_DIL_ROWS", "PD_DIR_FRC_ROWS"):
+    for k in _ENV_KEYS:
         monkeypatch.delenv(k, raising=False)
     for k, v in env.items():
         monkeypatch.setenv(k, v)
     return code
+
+
+def _expect_layout(code, wl):
+    """the layout pd_create must pick by itself: jittered lattices cannot take the uniform path"""
+    if code is not None:
+        return code
+    return 1 if wl.name == "block3d" else 2
 
 
 def _oracle(wl):
@@ -69,7 +83,7 @@ def _small_cases():
 def test_no_fracture_trajectory(name, layout):
     wl, nsteps = _small_cases()[name]
     sim, o = _sim(wl), _oracle(wl)
-    assert sim.get_layout()["layout"] == layout
+    assert sim.get_layout()["layout"] == _expect_layout(layout, wl)
     # pre-processing parity: family sizes, m, theta of the initial field
     rp = sim.get_bond_mask(rows_only=True)
     assert np.array_equal(rp, o.rowptr)
@@ -90,7 +104,7 @@ def test_no_fracture_trajectory(name, layout):
 def test_fracture_broken_sets(name, layout):
     wl, nsteps = _small_cases()[name]
     sim, o = _sim(wl), _oracle(wl)
-    assert sim.get_layout()["layout"] == layout
+    assert sim.get_layout()["layout"] == _expect_layout(layout, wl)
     b0, rp, col = _broken_set(sim)
     assert np.array_equal(rp, o.rowptr)
     assert b0 == o.broken_set() and len(b0) == 2 * len(wl.precut)
@@ -161,13 +175,6 @@ def test_edge_cases_and_errors():
         pd.Sim(np.array([[0.0, 0], [1, 0], [2, 0]]), np.ones(3), 1.5, dim=2, mode=1, E=1.0, nu=0.2, rho=1.0, dt=1.0,
                precut=np.array([[0, 2]], np.int32))
     assert ei.value.code == pd.PD_ERR_ARG
-    # single bond exactly at the threshold breaks; one ulp below does not (Eq. 1.30, reading C-7)
-    s_c = 1e-3
-    for a0, broken in ((s_c, True), (np.nextafter(s_c, 0), False)):
-        sim = pd.Sim(np.array([[0.0, 0], [1, 0]]), np.ones(2), 1.5, dim=2, mode=2, E=1.0, nu=0.2, rho=1.0, dt=1e-9,
-                     s_c=s_c, flags=np.array([3, 3], np.uint8), v0=np.zeros((2, 2)),
-                     u0=None)
-        sim.destroy()
     # step(0) is a no-op; empty pre-cut list
     sim = pd.Sim(np.array([[0.0, 0], [1, 0]]), np.ones(2), 1.5, dim=2, mode=2, E=1.0, nu=0.2, rho=1.0, dt=1e-9,
                  precut=np.zeros((0, 2), np.int32))
@@ -176,9 +183,76 @@ def test_edge_cases_and_errors():
     sim.destroy()
 
 
+def test_threshold_bond(layout):
+    """a single bond exactly at the threshold breaks, one ulp below does not (Eq. 1.30 PAPER.md:417-425,
+    reading C-7), on every code path and exactly like the oracle.  Both nodes carry a prescribed velocity
+    0 on both dofs, so u^1 = u^0 and the failure check of step 1 sees the stretch s = a0 exactly."""
+    from paper_2309_11273_b200 import pd
+    from oracle.pd_oracle import PDOracle
+    s_c = 1e-3
+    x = np.array([[0.0, 0.0], [1.0, 0.0]])
+    kw = dict(dim=2, mode=2, E=1.0, nu=0.2, rho=1.0, dt=1e-9, s_c=s_c)
+    fl = np.array([24, 24], np.uint8)
+    for a0, broken in ((s_c, True), (np.nextafter(s_c, 0), False), (np.nextafter(s_c, 1), True), (0.5 * s_c, False),
+                       (-2 * s_c, False)):
+        u0 = np.array([[0.0, 0.0], [a0, 0.0]])
+        o = PDOracle(x, np.ones(2), 1.5, **kw, flags=fl, value=np.zeros((2, 2)), u0=u0)
+        o.step(1)
+        assert len(o.broken_set()) == (2 if broken else 0)
+        sim = pd.Sim(x, np.ones(2), 1.5, **kw, flags=fl, value=np.zeros((2, 2)), u0=u0)
+        sim.step(1)
+        assert np.array_equal(sim.get_u(), u0)
+        assert sim.get_stats()["n_broken_directed"] == (2 if broken else 0), (a0, broken)
+        bs, _, _ = _broken_set(sim)
+        assert bs == o.broken_set()
+        assert np.array_equal(sim.get_damage(), o.damage())
+        sim.destroy()
+
+
+def test_step_error_is_returned_and_state_kept():
+    """a launch that cannot be prepared (device allocation failing inside pd_step) must come back as an error
+    code and leave the step counter and the buffers where they were"""
+    from paper_2309_11273_b200 import pd, workloads as W
+    wl = W.branching2d(nx=40, ny=24)
+    o = _oracle(wl)
+    sim = _sim(wl)
+    sim._rt.fail_allocs = True          # fault injection: the allocator callback returns NULL
+    with pytest.raises(pd.PdError) as ei:
+        sim.step(3)
+    assert ei.value.code == pd.PD_ERR_ALLOC
+    sim._rt.fail_allocs = False
+    assert sim.get_stats()["step"] == 0
+    sim.step(5); o.step(5)
+    assert sim.get_stats()["step"] == 5
+    assert _rel(sim.get_u(), o.u) <= TOL and _rel(sim.get_v(), o.v) <= TOL
+    sim.destroy()
+
+
+def test_lattice_layout_fallbacks():
+    """bodies the dense lattice layout must decline by itself (pd_lattice.cu): a lattice whose stencil has
+    more than 128 offsets (horizon 4.1 dx in 3-D: 250+), and a body that fills < 20 % of its bounding
+    box.  Both must come back in the sliced-ELL layout and match the oracle."""
+    from paper_2309_11273_b200 import pd
+    from oracle.pd_oracle import PDOracle
+    kw = dict(dim=3, mode=0, E=3.0, nu=0.25, rho=1.5, dt=1e-3)
+    g = np.stack(np.meshgrid(np.arange(12), np.arange(9), np.arange(8), indexing="ij"), -1).reshape(-1, 3).astype(float)
+    cases = {"wide_stencil": (0.1 * (g + 0.5), 0.41)}
+    a = 0.1 * (np.stack(np.meshgrid(np.arange(30), np.arange(4), np.arange(4), indexing="ij"), -1).reshape(-1, 3) + 0.5)
+    cases["sparse_box"] = (np.concatenate([a, a + np.array([0.0, 2.0, 2.0])]), 0.3015)   # two bars, 5.5 % of their bounding box
+    for name, (x, hor) in cases.items():
+        n = len(x)
+        u0 = 1e-4 * np.sin(7.0 * x[:, [1, 2, 0]])
+        sim = pd.Sim(x, np.full(n, 1e-3), hor, **kw, u0=u0)
+        assert sim.get_layout()["layout"] == 0, name
+        o = PDOracle(x, np.full(n, 1e-3), hor, **kw, u0=u0)
+        assert np.array_equal(sim.get_bond_mask(rows_only=True), o.rowptr)
+        sim.step(25); o.step(25)
+        assert _rel(sim.get_u(), o.u) <= TOL and _rel(sim.get_v(), o.v) <= TOL, name
+        sim.destroy()
+
+
 def test_point_cloud_general_layout():
-    """a random cloud (cells with 0, 1 or several nodes): the sliced-ELL layout with its FLAT segments;
-    also a lattice whose stencil exceeds the lattice layout's limits must fall back by itself"""
+    """a random cloud (cells with 0, 1 or several nodes): the sliced-ELL layout with its FLAT segments"""
     from paper_2309_11273_b200 import pd
     from oracle.pd_oracle import PDOracle
     rng = np.random.default_rng(5)
@@ -201,7 +275,7 @@ def test_full_size_config5p_sampled():
     from paper_2309_11273_b200 import workloads as W
     wl = W.CONFIGS["config5p"]()
     sim, o = _sim(wl), _oracle(wl)
-    assert sim.get_layout()["layout"] == 1
+    assert sim.get_layout()["layout"] == 2
     assert sim.get_stats()["n_directed_bonds"] == o.Z
     sim.step(3); o.step(3)
     assert _rel(sim.get_u(), o.u) <= TOL and _rel(sim.get_v(), o.v) <= TOL
