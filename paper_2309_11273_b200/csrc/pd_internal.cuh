@@ -119,6 +119,7 @@ struct PdLattice {
   double *uz[2] = {nullptr, nullptr};
   double2 *aux = nullptr;
   double *ctab[2] = {nullptr, nullptr};   // device: per stencil bit, the constants of the dilatation / force pass
+  void *ucols = nullptr;           // device: the column table of the uniform kernels
   int wbeg[5] = {0, 0, 0, 0, 0};   // columns whose bits lie in mask word w: wbeg[w] .. wbeg[w + 1] - 1
   int DX = 0, DY = 0, DZ = 0;      // dense dims incl. margins
   int HX = 0, HY = 0, HZ = 0;      // margins = stencil radius per axis

@@ -18,15 +18,18 @@ TOL = 1e-10
 # 1 = dense lattice with per-bond geometry (jittered config 4; PD_LAT_UNIFORM=0 forces it), 0 = sliced ELL.
 LAYOUTS = {
     "default": ({}, None),
-    # rows per lane swapped (2 in 3-D, 4 in 2-D), one prefetched record in the window, plain launches instead of graphs
-    "uniform_alt": ({"PD_ULAT_DIL_ROWS": "-1", "PD_ULAT_FRC_ROWS": "-1", "PD_ULAT_DIL_PF": "1", "PD_ULAT_FRC_PF": "1",
-                     "PD_GRAPH": "0"}, None),
+    # uniform lattice, records through L1 instead of TMA-staged planes; rows per lane swapped (2 in 3-D, 4 in 2-D);
+    # plain launches instead of CUDA graphs
+    "uniform_direct": ({"PD_ULAT_STAGED": "0", "PD_ULAT_DIL_ROWS": "-1", "PD_ULAT_FRC_ROWS": "-1", "PD_GRAPH": "0"}, None),
+    # staged planes with 3 buffers in flight, rows per lane swapped, 2 row groups per CTA
+    "uniform_nb3": ({"PD_ULAT_NB": "3", "PD_ULAT_DIL_ROWS": "-1", "PD_ULAT_FRC_ROWS": "-1", "PD_ULAT_DIL_CY": "2",
+                     "PD_ULAT_FRC_CY": "2"}, None),
     "lattice_general": ({"PD_LAT_UNIFORM": "0"}, 1),
     "lattice_general_2rows": ({"PD_LAT_UNIFORM": "0", "PD_DIR_DIL_ROWS": "2", "PD_DIR_FRC_ROWS": "2"}, 1),
     "sliced_ell": ({"PD_FORCE_GENERIC": "1"}, 0),
 }
 _ENV_KEYS = ("PD_LAT_UNIFORM", "PD_FORCE_GENERIC", "PD_DIR_DIL_ROWS", "PD_DIR_FRC_ROWS", "PD_ULAT_DIL_ROWS",
-             "PD_ULAT_FRC_ROWS", "PD_ULAT_DIL_PF", "PD_ULAT_FRC_PF", "PD_GRAPH")
+             "PD_ULAT_FRC_ROWS", "PD_ULAT_STAGED", "PD_ULAT_NB", "PD_ULAT_DIL_CY", "PD_ULAT_FRC_CY", "PD_GRAPH")
 
 
 @pytest.fixture(params=list(LAYOUTS))
