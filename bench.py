@@ -2,12 +2,21 @@
 """bench.py -- headline measurement of the OSB-PD explicit step on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config5|config5p|config4|config3|config2|config1]
+    python bench.py --workload all [--out profiles/r02_configs.json]   # the per-config table of DESIGN.md 5
     python bench.py --impl reference ...      # the CPU oracle as it stands, on the host cores
 
 A "step" is one pass of the whole hot path (dilatation(+break) kernel, force+update kernel: 2 launches)
 over the workload.  Metric (BASELINE.json): node-steps/s, FP64; bond-updates/s and the HBM roofline of
 the dominant kernel are in the same JSON line.  Default workload = config 5 (3D notched cylinder,
-3.144 M nodes, the config the >=60 %-of-HBM-roofline target is quoted on).
+3.144 M nodes, the config the >=60 %-of-HBM-roofline target is quoted on), default step count = the
+workload's STATED step count (W warm-up steps + K timed steps = 2000 for config 5), so the timed window
+holds the fracture phase of the run (state.broken_directed is printed at the start and at the end).
+
+Timing protocol: pass 1 advances a fresh handle W steps untimed, then exactly K steps between two CUDA
+events on the stream the kernels are launched on (-> value, ms_per_step).  Pass 2 repeats the same W + K
+steps on a second fresh handle with CUDA events around every launch (-> per-kernel durations over the same
+K steps -> roofline).  Inputs are larger than L2 for configs 4, 5, 5' (no flush needed); configs 1-3 fit L2
+and say so.
 
 N > 1 (torchrun, one rank per GPU): the path is not sharded ("replicas only"), every
 rank advances an independent replica of the workload; value = N * nodes * K / max-over-ranks time.
@@ -15,6 +24,7 @@ rank advances an independent replica of the workload; value = N * nodes * K / ma
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import subprocess
@@ -29,6 +39,8 @@ if ROOT not in sys.path:
 import numpy as np  # noqa: E402
 
 METRIC = "node-steps/s"
+ALL = ["config1", "config2", "config3", "config4", "config5p", "config5"]
+FP64_PEAK = 148 * 64 * 1.965e9   # FP64 lanes x SMs x max SM clock: warp-wide FP64 instructions retire at 2 per clock and SM
 
 
 def make_workload(name):
@@ -42,6 +54,21 @@ def byte_model(n, z, dim, fracture):
     dil = 4.125 * z + n * (16 * dim + 28 + (8 if fracture else 0))
     frc = 4.125 * z + n * (40 * dim + 29)
     return dil, frc
+
+
+# FP64 instructions the arithmetic of the shipped kernels needs per directed bond (dilatation, force), by layout
+# (counted in the SASS of the FAST step: profiles/r02_kernels.md)
+FP64_PER_BOND = {2: (7.0, 12.5), 1: (10.0, 22.0), 0: (10.0, 22.0)}
+
+
+def kernel_source_hash():
+    """sha256 over the CUDA sources: ncu traffic figures are only quoted for the build they were captured on"""
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2309_11273_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
 
 
 class ClockSampler(threading.Thread):
@@ -86,15 +113,15 @@ class ClockSampler(threading.Thread):
         return out
 
 
-def oracle_sample(wl_name, steps):
+def oracle_sample(wl_name):
     """bounded sample of the benchmark workload for the CPU oracle: same cross-section / lattice,
     material, dt, boundary recipe; fewer nodes and steps (about 10-30 s of CPU work)."""
     from paper_2309_11273_b200 import workloads as W
     if wl_name in ("config5", "config5p"):
-        return W.cylinder3d(r_cells=50, l_cells=16), "r=50 cells (full cross-section), L=16 cells = 125 760 nodes", steps
+        return W.cylinder3d(r_cells=50, l_cells=16), "SAMPLE of the workload: r=50 cells (full cross-section), L=16 cells = 125 760 nodes"
     if wl_name == "config4":
-        return W.block3d(nx=80, ny=40, nz=40), "80x40x40 = 128 000 nodes", steps
-    return W.CONFIGS[wl_name](), "full workload", steps
+        return W.block3d(nx=80, ny=40, nz=40), "SAMPLE of the workload: 80x40x40 = 128 000 nodes"
+    return W.CONFIGS[wl_name](), "full workload"
 
 
 def time_oracle(wl, steps):
@@ -107,20 +134,35 @@ def time_oracle(wl, steps):
     return wl.n * steps / dt, dt, o.Z, pd_oracle.num_threads()
 
 
+def oracle_single_thread(wl_name, steps):
+    """node-steps/s of the oracle on ONE host core (SURVEY 8(d) "oracle timing (i)"): a child process with
+    OMP_NUM_THREADS=1 (the thread count of an OpenMP runtime is fixed when the library is loaded)"""
+    code = ("import json,sys; sys.path.insert(0, %r); import bench; wl, _ = bench.oracle_sample(%r); "
+            "v, dt, z, c = bench.time_oracle(wl, %d); print(json.dumps({'value': v, 'seconds': dt, 'cores': c}))"
+            % (ROOT, wl_name, steps))
+    try:
+        out = subprocess.run([sys.executable, "-c", code], env=dict(os.environ, OMP_NUM_THREADS="1"), capture_output=True,
+                             text=True, timeout=600)
+        return json.loads(out.stdout.strip().splitlines()[-1])
+    except Exception:
+        return None
+
+
 def run_reference(args):
     from paper_2309_11273_b200 import replicas
     if replicas.rank_info()[0] != 0:   # under torchrun rank 0 alone runs and prints the reference arm
         return 0
-    wl, desc, _ = oracle_sample(args.workload, args.steps)
-    per_step = max(1, min(args.steps, 50 if wl.dim == 3 else 500))
+    name = "config5" if args.workload == "all" else args.workload
+    wl, desc = oracle_sample(name)
+    k = args.steps if args.steps else 50
+    per_step = max(1, min(k, 50 if wl.dim == 3 else 500))
     time_oracle(wl, max(1, min(args.warmup, 1)))          # warm-up (page in, build the .so)
-    t0 = time.perf_counter()
     val, dt, z, cores = time_oracle(wl, per_step)
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": "node-steps/s", "n_gpus": args.gpus,
         "steps": per_step, "warmup": 1, "ms_per_step": 1e3 * dt / per_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "sample": desc, "nodes": wl.n, "directed_bonds": z},
+        "config": {"workload": name, "sample": desc, "nodes": wl.n, "directed_bonds": z},
         "bond_updates_per_s": z * per_step / dt,
         "cpu_baseline": {"value": val, "unit": "node-steps/s", "cores": cores, "kind": "oracle",
                          "sample": f"{desc}, {per_step} steps"},
@@ -130,39 +172,15 @@ def run_reference(args):
     return 0
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=300)
-    ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config5")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    args = ap.parse_args()
-    if args.impl == "reference":
-        return run_reference(args)
-
+def measure(name, K, Wm, local, world, want_e2e, want_cpu):
+    """one workload on this rank -> the JSON line (rank 0) or None"""
     import torch
     import torch.distributed as dist
-    from paper_2309_11273_b200 import pd
-
-    from paper_2309_11273_b200 import replicas
-    rank, local, world = replicas.rank_info()
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    K, Wm = args.steps, max(args.warmup, 3)
-
-    wl = make_workload(args.workload)
-    t0 = time.perf_counter()
-    sim = pd.Sim.from_workload(wl, device=f"cuda:{local}")
-    torch.cuda.synchronize()
-    t_build = time.perf_counter() - t0
-    lay = sim.get_layout()
-    n, z = lay["n"], lay["n_directed_bonds"]
+    from paper_2309_11273_b200 import pd, replicas
+    rank = replicas.rank_info()[0]
+    wl = make_workload(name)
+    if K is None:
+        K = max(1, wl.steps - Wm)       # W + K = the workload's stated step count
     fracture = wl.s_c > 0
 
     def barrier():
@@ -170,8 +188,15 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident timing: W warm-up steps, then exactly K steps between CUDA events ----
+    # ---- pass 1: W warm-up steps, then exactly K steps between CUDA events ----
+    t0 = time.perf_counter()
+    sim = pd.Sim.from_workload(wl, device=f"cuda:{local}")
+    torch.cuda.synchronize()
+    t_build = time.perf_counter() - t0
+    lay = sim.get_layout()
+    n, z = lay["n"], lay["n_directed_bonds"]
     sim.step(Wm)
+    broken0 = sim.get_stats()["n_broken_directed"]
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
@@ -187,19 +212,21 @@ def main():
     tw1 = time.time()
     ms = ev0.elapsed_time(ev1)
     launches = sim.get_layout()["step_launches"] - l0
-    # ---- per-kernel durations (events around every launch), same state, K more steps ----
-    kd, kf = sim.step_timed(min(K, 100))
-    nk = min(K, 100)
     sampler.stop()
     clocks = sampler.summary(tw0, tw1)
     ms = replicas.max_over_ranks(ms, device="cuda")
     stats = sim.get_stats()
     u_max = float(np.abs(sim.get_u()).max()) if rank == 0 else 0.0
     sim.destroy()
+    # ---- pass 2: the same W + K steps with CUDA events around every launch: per-kernel durations ----
+    sim = pd.Sim.from_workload(wl, device=f"cuda:{local}")
+    sim.step(Wm)
+    kd, kf = sim.step_timed(K)
+    sim.destroy()
 
     # ---- end-to-end through the C-ABI with HOST buffers (create + K steps + read-back, all timed) ----
     e2e = None
-    if not args.no_e2e:
+    if want_e2e:
         host = {k: np.ascontiguousarray(getattr(wl, k)) for k in ("coords", "volumes", "flags", "value", "precut", "u0", "v0")}
         h2d = sum(a.nbytes for a in host.values())
         barrier()
@@ -216,11 +243,8 @@ def main():
         e2e = {"value": replicas.whole_job_throughput(n, K, te * 1e3, world), "unit": "node-steps/s", "h2d_bytes_per_step": h2d / K,
                "d2h_bytes_per_step": d2h / K, "seconds": te,
                "note": "pd_create from host arrays (family build included) + pd_step(K) + pd_get_u/v/damage to host"}
-
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return 0
+        return None
 
     peaks = {}
     try:
@@ -230,53 +254,112 @@ def main():
     peak = float(peaks.get("hbm_gbs", 6650.0))
     peak_kind = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
     b_dil, b_frc = byte_model(n, z, wl.dim, fracture)
-    traffic = {}
-    try:   # DRAM bytes per launch of the two kernels from the committed ncu capture (profiles/r01c_direct_kernels.md)
-        traffic = json.load(open(os.path.join(ROOT, "profiles", "r01c_traffic.json"))).get(args.workload, {})
+    # DRAM bytes per launch from the committed ncu capture -- only if it was taken on exactly this kernel source
+    traffic, traffic_note = {}, "no ncu capture for this workload"
+    try:
+        tj = json.load(open(os.path.join(ROOT, "profiles", "r02_traffic.json")))
+        if tj.get("kernel_source_sha") != kernel_source_hash():
+            traffic_note = "stale: the ncu capture in profiles/r02_traffic.json is of another build of the kernels"
+        elif lay.get("layout") != tj.get("layout", {}).get(name):
+            traffic_note = "the ncu capture is of another layout"
+        else:
+            traffic, traffic_note = tj.get(name, {}), tj.get("unit", "")
     except Exception:
         pass
-    if lay.get("layout") != 1:
-        traffic = {}   # the capture is of the default (lattice / direct) kernels
-    t_dil, t_frc = kd / nk * 1e-3, kf / nk * 1e-3
+    t_dil, t_frc = kd / K * 1e-3, kf / K * 1e-3
     dom = ("k_force_update", b_frc, t_frc) if t_frc >= t_dil else ("k_dilatation", b_dil, t_dil)
     achieved = dom[1] / dom[2] / 1e9
     step_s = ms * 1e-3 / K
+    fp_d, fp_f = FP64_PER_BOND.get(lay.get("layout"), (10.0, 22.0))
+    l2 = 4 * z > 2 * 126e6
+    tr = traffic.get(dom[0])
     line = {
         "metric": METRIC, "value": replicas.whole_job_throughput(n, K, ms, world), "unit": "node-steps/s", "n_gpus": world, "steps": K,
         "warmup": Wm, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{args.workload}:{wl.name}", "nodes": n, "directed_bonds": z, "dim": wl.dim,
-                   "fracture": bool(fracture), "horizon_over_dx": 3.015, "l2": "inputs larger than L2 (no flush needed)"
-                   if 4 * z > 2 * 126e6 else "working set fits L2: HBM fraction not meaningful", "parallelism":
-                   "replicas only" if world > 1 else "1 GPU", "build_seconds": t_build, "layout": lay},
+        "config": {"workload": f"{name}:{wl.name}", "nodes": n, "directed_bonds": z, "dim": wl.dim,
+                   "fracture": bool(fracture), "stated_steps": wl.steps, "horizon_over_dx": 3.015,
+                   "l2": "inputs larger than L2 (no flush needed)" if l2 else "working set fits L2: HBM fraction not meaningful",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU", "build_seconds": t_build, "layout": lay},
         "bond_updates_per_s": replicas.whole_job_throughput(z, K, ms, world),
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": {"bound": "hbm", "kernel": dom[0], "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": traffic.get(dom[0]), "peak_kind": peak_kind,
-                     "algorithmic_bytes_per_launch": dom[1], "kernel_ms": dom[2] * 1e3},
+                     "frac": achieved / peak, "traffic": tr, "traffic_note": traffic_note,
+                     "actual_dram_GBps": (tr / dom[2] / 1e9) if tr else None, "peak_kind": peak_kind,
+                     "algorithmic_bytes_per_launch": dom[1], "kernel_ms": dom[2] * 1e3,
+                     "kernel_ms_is": "mean over the K timed steps, CUDA events around every launch (pass 2)"},
         "kernels": {"k_dilatation": {"ms": t_dil * 1e3, "algorithmic_bytes": b_dil, "GBps": b_dil / t_dil / 1e9},
                     "k_force_update": {"ms": t_frc * 1e3, "algorithmic_bytes": b_frc, "GBps": b_frc / t_frc / 1e9}},
-        # co-limiter: FP64 instructions the arithmetic of the method needs per directed bond
-        # (10 dilatation [14 with the exact break test], 22 force) against 148 SM x 64 FP64 lanes x 1.965 GHz
-        "fp64_roofline": {"bound": "alu", "kernel": "k_force_update", "achieved": 22.0 * z / t_frc / 1e12,
-                          "peak": 148 * 64 * 1.965e9 / 1e12, "unit": "T FP64 instr/s",
-                          "frac": 22.0 * z / t_frc / (148 * 64 * 1.965e9),
-                          "step_frac": (10.0 + 22.0) * z / step_s / (148 * 64 * 1.965e9)},
+        # co-limiter: FP64 instructions the arithmetic of the shipped kernels needs per directed bond
+        "fp64_roofline": {"bound": "alu", "kernel": dom[0], "fp64_per_bond": {"k_dilatation": fp_d, "k_force_update": fp_f},
+                          "achieved": (fp_f if dom[0] == "k_force_update" else fp_d) * z / dom[2] / 1e12,
+                          "peak": FP64_PEAK / 1e12, "unit": "T FP64 instr/s",
+                          "frac": (fp_f if dom[0] == "k_force_update" else fp_d) * z / dom[2] / FP64_PEAK,
+                          "step_frac": (fp_d + fp_f) * z / step_s / FP64_PEAK},
         "step_roofline": {"algorithmic_bytes_per_step_B2": b_dil + b_frc, "achieved_GBps": (b_dil + b_frc) / step_s / 1e9,
                           "frac_of_peak": (b_dil + b_frc) / step_s / 1e9 / peak, "frac_of_8TBps_nominal":
                           (b_dil + b_frc) / step_s / 8e12},
-        "state": {"broken_directed": stats["n_broken_directed"], "max_damage": stats["max_damage"], "max_abs_u": u_max},
+        "state": {"broken_directed_at_start_of_timed_window": broken0, "broken_directed": stats["n_broken_directed"],
+                  "max_damage": stats["max_damage"], "nodes_damage_ge_half": stats["n_nodes_damage_ge_half"],
+                  "step": stats["step"], "max_abs_u": u_max},
     }
     if e2e:
         line["e2e"] = e2e
-    if not args.no_cpu_baseline:
-        swl, desc, _ = oracle_sample(args.workload, K)
+    if want_cpu:
+        swl, desc = oracle_sample(name)
         osteps = 600 if swl.dim == 3 else 4000   # about 10-20 s of CPU work
         val, dt, zz, cores = time_oracle(swl, osteps)
         line["cpu_baseline"] = {"value": val, "unit": "node-steps/s", "cores": cores, "kind": "oracle",
                                 "sample": f"{desc}, {osteps} steps, {dt:.1f} s"}
-    print(json.dumps(line))
+        one = oracle_single_thread(name, 40 if swl.dim == 3 else 400)
+        if one:
+            line["cpu_baseline"]["single_thread"] = {"value": one["value"], "cores": one["cores"], "seconds": one["seconds"]}
+    return line
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None, help="timed steps K (default: stated steps of the workload - warmup)")
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config5")
+    ap.add_argument("--out", default=None, help="--workload all: write the per-config records to this JSON file")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2309_11273_b200 import replicas
+    rank, local, world = replicas.rank_info()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    Wm = max(args.warmup, 3)
+
+    if args.workload == "all":
+        recs = []
+        for name in ALL:
+            line = measure(name, args.steps, Wm, local, world, False, False)
+            if line:
+                recs.append(line)
+        if rank == 0:
+            out = {"kernel_source_sha": kernel_source_hash(), "records": recs}
+            if args.out:
+                with open(args.out, "w") as f:
+                    json.dump(out, f, indent=1)
+            print(json.dumps({"metric": METRIC, "workload": "all", "records": [
+                {"workload": r["config"]["workload"], "ms_per_step": r["ms_per_step"], "value": r["value"]} for r in recs]}))
+    else:
+        line = measure(args.workload, args.steps, Wm, local, world, not args.no_e2e, not args.no_cpu_baseline)
+        if line:
+            print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
     return 0

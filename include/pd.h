@@ -43,7 +43,9 @@ extern "C" {
 #define PD_ERR_ISOLATED (-2) /* a node has an empty family (m_i = 0 would divide by zero, Eq. 1.6)     */
 #define PD_ERR_ALLOC (-3)    /* device allocation failed                                               */
 #define PD_ERR_CUDA (-4)     /* CUDA runtime error / no device                                         */
-#define PD_ERR_LIMIT (-5)    /* problem exceeds an internal limit (2^31 directed bonds, cell table)    */
+#define PD_ERR_LIMIT (-5)    /* problem exceeds an internal limit (2^31 directed bonds, cell table).
+                                (SURVEY 8(b) sketched -5 as "non-finite state, debug builds"; there is no debug
+                                build of this library, so the code is used for limits: DESIGN.md 1)      */
 
 /* dimension modes: constants A, K, G of Eqs. 1.8, 1.15, 1.16 */
 #define PD_MODE_3D 0
@@ -118,12 +120,22 @@ PD_API int pd_create(pd_sim **out, int64_t n, const double *coords, const double
  *  (5) every intact bond with s_ij = e_ij(u^{n+1})/xbar_ij >= s_c breaks, irreversibly
  *      (Eqs. 1.17, 1.30); damage phi_i = 1 - sum_j rho_ij V_j / sum_j V_j (Eq. 1.31)
  * Observable state at step boundaries is (u^n, v^n, rho^n, phi^n): forces at step n use rho^n
- * and u^n; rho^{n+1} is decided from u^{n+1}.  Asynchronous; errors surface in the next
- * synchronising call.
+ * and u^n; rho^{n+1} is decided from u^{n+1}.  Asynchronous: no host synchronisation; in the steady
+ * state (load ramp finished) the steps are replayed from a CUDA graph captured once per handle.
+ * A launch that cannot be prepared returns its error code and leaves the step counter and the state
+ * where they were; errors of the device work itself surface in the next synchronising call.
  */
 PD_API int pd_step(pd_sim *sim, int64_t nsteps);
 
-/* dst: dim*n doubles (u, v) / n doubles (damage), user order, host or device.  Synchronise. */
+/*
+ * pd_get_u / pd_get_v -- the state of the explicit scheme at the current step boundary: displacement u^n and
+ * velocity v^n of Eq. 2.11 (`U`, `VEL` of App. A/B).
+ *   dst  dim*n doubles, AoS, user node order, host or device, caller-owned.
+ * pd_get_damage -- phi_i = 1 - sum_j rho_ij V_j / sum_j V_j (Eq. 1.31) with rho^n decided from u^n
+ * (Eq. 1.30; a deferred failure pass is flushed first), denominator over the full geometric family.
+ *   dst  n doubles, user node order, host or device, caller-owned.
+ * All three synchronise with the stream.  Errors: PD_ERR_ARG (null), PD_ERR_ALLOC, PD_ERR_CUDA.
+ */
 PD_API int pd_get_u(pd_sim *sim, double *dst);
 PD_API int pd_get_v(pd_sim *sim, double *dst);
 PD_API int pd_get_damage(pd_sim *sim, double *dst);
@@ -149,8 +161,9 @@ PD_API int pd_get_node_fields(pd_sim *sim, double *m, double *theta);
 /* layout/launch facts for the roofline report: counts[0]=n, [1]=n padded (array length incl. phantoms),
  * [2]=Z directed bonds, [3]=stored neighbour-index slots (0 in the lattice layout, which stores none),
  * [4]=kernel launches issued by pd_step so far, [5]=bytes of device memory held, [6]=1 if volumes are
- * uniform, [7]=layout: 0 = windowed sliced ELL (any point cloud), 1 = dense lattice / direct kernels,
- * 2 = dense lattice / shared-memory marching kernels. */
+ * uniform, [7]=layout: 0 = windowed sliced ELL (any point cloud), 1 = dense lattice, bond geometry per bond
+ * (jittered lattices), 2 = dense UNIFORM lattice, bond geometry a constant per stencil offset (the paper's
+ * uniform grids). */
 PD_API int pd_get_layout(pd_sim *sim, int64_t counts[8]);
 
 /* measurement aid for the roofline report: like pd_step, but brackets every kernel launch with

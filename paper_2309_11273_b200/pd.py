@@ -84,7 +84,8 @@ def _ptr(a):
 
 
 class _TorchRuntime:
-    """pd_runtime backed by torch's caching allocator and current stream."""
+    """pd_runtime backed by torch's caching allocator and the stream that is current when the handle is created
+    (the handle keeps that stream for its whole life: pd_runtime is read once, in pd_create)."""
 
     def __init__(self, device):
         import torch
@@ -121,6 +122,8 @@ class Sim:
             raise RuntimeError("no CUDA device: paper_2309_11273_b200 has no CPU path")
         self.lib = load()
         self.device = torch.device(device)
+        if self.device.index is None:
+            self.device = torch.device("cuda", torch.cuda.current_device())
         torch.cuda.set_device(self.device)
         self.dim = int(dim)
         keep = []
@@ -181,6 +184,16 @@ class Sim:
     def _get(self, fn, shape, out):
         if out is None:
             out = np.empty(shape, dtype=np.float64)
+        else:   # the library writes prod(shape) doubles through the raw pointer: refuse anything else
+            n = int(np.prod(shape))
+            if isinstance(out, np.ndarray):
+                ok = out.dtype == np.float64 and out.flags["C_CONTIGUOUS"] and out.size == n
+            else:   # torch tensor: host, or on this handle's device
+                import torch
+                ok = (out.dtype == torch.float64 and out.is_contiguous() and out.numel() == n and
+                      (not out.is_cuda or out.device == self.device))
+            if not ok:
+                raise ValueError(f"out must be a contiguous float64 array of {n} elements on the host or on {self.device}")
         self._ck(fn(self.h, _ptr(out)))
         return out
 

@@ -302,6 +302,24 @@ def test_single_bond_breaks_at_threshold():
     assert o.break_bonds()[0] == 0
 
 
+def test_near_threshold_counter():
+    """the oracle's near-threshold counter (north star: bonds within 1e-9 relative of s_c at the step they
+    break "are counted and reported"): a bond at s_c (1 +- 5e-10) is counted (in both directions), one at
+    s_c (1 +- 1e-8) is not; the counter is independent of whether the bond breaks; step() accumulates it"""
+    s_c = 1e-3
+    for rel, near in [(+5e-10, 2), (-5e-10, 2), (+1e-8, 0), (-1e-8, 0), (0.0, 2)]:
+        a = s_c * (1.0 + rel)
+        o = make([[0, 0], [1, 0]], 2, MODE_PLANE_STRAIN, 1.5, s_c=s_c, u0=np.array([[0, 0], [a, 0.0]]))
+        nb, nn = o.break_bonds(near_tol=1e-9)
+        assert nn == near, (rel, nn)
+        assert nb == (2 if rel >= 0 else 0)
+    # through the time stepper: both dofs of both nodes carry a prescribed velocity 0, so u^1 = u^0
+    a = s_c * (1.0 - 5e-10)
+    o = make([[0, 0], [1, 0]], 2, MODE_PLANE_STRAIN, 1.5, s_c=s_c, u0=np.array([[0, 0], [a, 0.0]]),
+             flags=np.array([24, 24], np.uint8), value=np.zeros((2, 2)), dt=1e-9)
+    assert o.step(3) == 0 and o.near_total == 6   # 2 directed bonds x 3 steps, never breaking
+
+
 def test_damage_half_family_and_precut_band():
     x = lattice((9, 9))
     o = make(x, 2, MODE_PLANE_STRESS, 3.015)
