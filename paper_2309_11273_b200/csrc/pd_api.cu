@@ -243,6 +243,9 @@ int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volum
   if (e != cudaSuccess) return fail(pdi::cuda_fail(e, "pd_create state initialisation"));
   for (void *p : {d_coords, d_vol, d_flags, d_precut, d_u0, d_v0, d_val}) pdi::dev_free(s, p);
   s->cur = 0; s->step = 0; s->break_pending = false;  // u^0 is not break-checked (reading C-5)
+  // graphs pay where the step is launch-bound (the 2-D configs: 10-20 us of kernel time per step); with more than
+  // 2e7 directed bonds a launch is 0.1 ms and longer and the plain launches cost nothing
+  s->use_graph = s->Z < 20000000;
   if (const char *env = getenv("PD_GRAPH")) s->use_graph = atoi(env) != 0;
   if (const char *env = getenv("PD_GRAPH_STEPS")) s->graph_len = std::max(2, std::min(atoi(env) & ~1, 256));
   *out = s;
@@ -303,7 +306,9 @@ int pd_step(pd_sim *s, int64_t nsteps) {
       const int which = (left >= big && big > 2) ? 1 : 0;
       const int len = which ? big : 2;
       if (!s->graph[which] && !s->graph_failed) {
-        if (s->step < 4) {   // the first steps run by plain launches (they also prepare the launch arguments)
+        // the first steps run by plain launches (they also prepare the launch arguments); a graph is only built
+        // when enough steps are left to pay for its instantiation
+        if (s->step < 4 || left < 64) {
           if (int rc = step_once(s)) return rc;
           --left;
           continue;
