@@ -41,13 +41,18 @@ def weighted_volume(n, bonds, xi, vol):
     return m
 
 
-def pd_force(U, vol, bonds, m, xi, Xi, co_index, A, K, G):
+def pd_force(U, vol, bonds, m, xi, Xi, co_index, A, K, G, geometric=False):
     """PDForceComputLoop of App. C (vectorised over bonds; np.add.at plays the loop).
-    U: (Nn, dim).  Returns PDF (Nn, dim) nodal forces and Theta."""
+    U: (Nn, dim).  Returns PDF (Nn, dim) nodal forces and Theta.
+    geometric=True keeps the extension exactly as the listing prints it."""
     n, dim = U.shape
     i1, i2 = bonds[:, 0], bonds[:, 1]
     M = Xi / xi[:, None]
-    E = np.sum(M * (U[i2] - U[i1]), axis=1)          # linearized (Eq. 2.7)
+    if geometric:
+        Eta = Xi + (U[i2] - U[i1])                   # PAPER.md:908-910
+        E = np.sqrt(np.sum(Eta * Eta, axis=1)) - xi  # PAPER.md:911-912
+    else:
+        E = np.sum(M * (U[i2] - U[i1]), axis=1)      # linearized (Eq. 2.7)
     E = np.where(co_index == 0, 0.0, E)              # PAPER.md:913
     theta = np.zeros(n)
     np.add.at(theta, i1, A * xi * E * co_index * vol[i2])   # PAPER.md:917

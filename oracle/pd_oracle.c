@@ -495,3 +495,87 @@ int64_t pdo_run(int64_t n, int dim, const double *coords, const double *V, const
   free(before);
   return total;
 }
+
+/* ==========================================================================================
+ * VARIANT: the GEOMETRIC extension of the paper's own loop code,
+ *   e_ij = || xi_ij + eta_ij || - || xi_ij ||,  eta_ij = u_j - u_i       (App. C),
+ * used in place of the linearized M . eta in the dilatation, the force AND the failure stretch
+ * s = e / xbar; the direction stays M = xi / xbar (App. C).  Everything else
+ * (steps 7, 8, 9, 11) is the code above, unchanged.  Evaluation order as in the listing:
+ * Eta_k = Xi_k + (U_j,k - U_i,k), eta = sqrt(sum_k Eta_k^2) summed in k order, E = eta - xi.
+ * Pins (tests/test_oracle_pins.py): a FINITE rigid rotation gives e = 0 and zero force (the linearized
+ * model does not), transverse hand value sqrt(r^2 + b^2) - r, e_geo -> e_lin quadratically for small
+ * eta, the App. C pair-scatter code with its printed (geometric) extension.
+ * ======================================================================================== */
+void pdo_extension_geom(int64_t n, int dim, const double *coords, const int64_t *rowptr,
+                        const int32_t *col, const uint8_t *rho, const double *u, double *e,
+                        double *xbar_out) {
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < n; ++i) {
+    for (int64_t p = rowptr[i]; p < rowptr[i + 1]; ++p) {
+      int64_t j = col[p];
+      double xbar = sqrt(dist2(dim, coords + dim * i, coords + dim * j));
+      double s = 0.0;
+      for (int k = 0; k < dim; ++k) {
+        double Eta = (coords[dim * j + k] - coords[dim * i + k]) + (u[dim * j + k] - u[dim * i + k]);
+        s += Eta * Eta;
+      }
+      double ext = sqrt(s) - xbar;
+      e[p] = rho[p] ? ext : 0.0;
+      if (xbar_out) xbar_out[p] = xbar;
+    }
+  }
+}
+
+int64_t pdo_break_geom(int64_t n, int dim, const double *coords, const int64_t *rowptr,
+                       const int32_t *col, const uint8_t *flags, const double *u, double s_c,
+                       uint8_t *rho, double near_tol, int64_t *near) {
+  int64_t broken = 0, nnear = 0;
+#pragma omp parallel for schedule(static) reduction(+ : broken, nnear)
+  for (int64_t i = 0; i < n; ++i) {
+    for (int64_t p = rowptr[i]; p < rowptr[i + 1]; ++p) {
+      if (!rho[p]) continue;
+      int64_t j = col[p];
+      double xbar = sqrt(dist2(dim, coords + dim * i, coords + dim * j));
+      double sq = 0.0;
+      for (int k = 0; k < dim; ++k) {
+        double Eta = (coords[dim * j + k] - coords[dim * i + k]) + (u[dim * j + k] - u[dim * i + k]);
+        sq += Eta * Eta;
+      }
+      double s = (sqrt(sq) - xbar) / xbar;
+      if (fabs(s - s_c) <= near_tol * s_c) ++nnear;
+      int nofail = flags && ((flags[i] | flags[j]) & PDO_NOFAIL);
+      if (s >= s_c && !nofail) {
+        rho[p] = 0;
+        ++broken;
+      }
+    }
+  }
+  if (near) *near = nnear;
+  return broken;
+}
+
+/* the whole step with the geometric extension: pdo_run with steps 6 and 10 replaced */
+int64_t pdo_run_geom(int64_t n, int dim, const double *coords, const double *V, const int64_t *rowptr,
+                     const int32_t *col, uint8_t *rho, const double *m, const double *fvol,
+                     const uint8_t *flags, const double *bval, double A, double K, double G,
+                     double rho_mass, double dt, double ramp_time, double s_c, int64_t step0,
+                     int64_t nsteps, double *u, double *v, double *phi, double *e, double *xbar,
+                     double *theta, double *f, double near_tol, int64_t *near_total) {
+  int fracture = (s_c > 0.0) && isfinite(s_c);
+  int64_t total = 0, near_sum = 0;
+  for (int64_t s = 0; s < nsteps; ++s) {
+    pdo_extension_geom(n, dim, coords, rowptr, col, rho, u, e, xbar);
+    pdo_dilatation(n, V, rowptr, col, e, xbar, A, m, theta);
+    pdo_force_density(n, dim, coords, V, rowptr, col, rho, e, xbar, theta, m, K, G, f);
+    pdo_update(n, dim, f, flags, bval, rho_mass, dt, ramp_time, step0 + s, u, v);
+    if (fracture) {
+      int64_t nn = 0;
+      total += pdo_break_geom(n, dim, coords, rowptr, col, flags, u, s_c, rho, near_tol, &nn);
+      near_sum += nn;
+    }
+  }
+  if (phi) pdo_damage(n, V, rowptr, col, rho, fvol, phi);
+  if (near_total) *near_total = near_sum;
+  return total;
+}

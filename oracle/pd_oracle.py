@@ -44,6 +44,8 @@ def lib():
         _lib.pdo_find_bond.restype = C.c_int64
         _lib.pdo_break.restype = C.c_int64
         _lib.pdo_run.restype = C.c_int64
+        _lib.pdo_run_geom.restype = C.c_int64
+        _lib.pdo_break_geom.restype = C.c_int64
         _lib.pdo_num_threads.restype = C.c_int
     return _lib
 
@@ -97,7 +99,9 @@ class PDOracle:
 
     def __init__(self, coords, volumes, horizon, *, dim, mode, E, nu, rho, dt, s_c=0.0,
                  ramp_time=0.0, flags=None, value=None, precut=None, u0=None, v0=None,
-                 family_method="cells"):
+                 family_method="cells", extension="linearized"):
+        assert extension in ("linearized", "geometric")   # geometric: App. C's e = ||xi+eta|| - ||xi||
+        self.geom = extension == "geometric"
         self.coords = _f64(coords).reshape(-1, dim)
         self.n, self.dim = self.coords.shape
         self.V = _f64(volumes).reshape(self.n)
@@ -146,7 +150,8 @@ class PDOracle:
     # ---- pieces (used by the pins) ------------------------------------------------------
     def extension(self, u=None):
         u = self.u if u is None else _f64(u, (self.n, self.dim))
-        lib().pdo_extension(C.c_int64(self.n), C.c_int(self.dim), _p(self.coords), _p(self.rowptr),
+        fn = lib().pdo_extension_geom if self.geom else lib().pdo_extension
+        fn(C.c_int64(self.n), C.c_int(self.dim), _p(self.coords), _p(self.rowptr),
                             _p(self.col), _p(self.rho), _p(u), _p(self.e), _p(self.xbar))
         return self.e
 
@@ -174,7 +179,8 @@ class PDOracle:
 
     def break_bonds(self, near_tol=1e-9):
         near = C.c_int64(0)
-        nb = lib().pdo_break(C.c_int64(self.n), C.c_int(self.dim), _p(self.coords), _p(self.rowptr),
+        fn = lib().pdo_break_geom if self.geom else lib().pdo_break
+        nb = fn(C.c_int64(self.n), C.c_int(self.dim), _p(self.coords), _p(self.rowptr),
                              _p(self.col), _p(self.flags), _p(self.u), C.c_double(self.s_c),
                              _p(self.rho), C.c_double(near_tol), C.byref(near))
         return int(nb), int(near.value)
@@ -186,6 +192,18 @@ class PDOracle:
 
     # ---- the time step ------------------------------------------------------------------
     def step(self, nsteps: int, log_breaks: bool = False, near_tol: float = 1e-9) -> int:
+        if self.geom:
+            near = C.c_int64(0)
+            nb = lib().pdo_run_geom(
+                C.c_int64(self.n), C.c_int(self.dim), _p(self.coords), _p(self.V), _p(self.rowptr),
+                _p(self.col), _p(self.rho), _p(self.m), _p(self.fvol), _p(self.flags), _p(self.value),
+                C.c_double(self.A), C.c_double(self.K), C.c_double(self.G), C.c_double(self.rho_mass),
+                C.c_double(self.dt), C.c_double(self.ramp_time), C.c_double(self.s_c),
+                C.c_int64(self.step_index), C.c_int64(nsteps), _p(self.u), _p(self.v), _p(self.phi),
+                _p(self.e), _p(self.xbar), _p(self.theta), _p(self.f), C.c_double(near_tol), C.byref(near))
+            self.step_index += nsteps
+            self.near_total += int(near.value)
+            return int(nb)
         near = C.c_int64(0)
         logn = C.c_int64(0)
         cap = 0

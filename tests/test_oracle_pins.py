@@ -392,3 +392,68 @@ def test_critical_stretch_and_literals():
         assert row["dt"] < 0.81 * row["dt_crit"] and row["dt_crit"] < row["delta_over_c"]  # reading C-8
     assert workloads.SCALARS["branching2d"]["s_c"] == pytest.approx(
         scalars.critical_stretch(MODE_PLANE_STRESS, 72e9, 0.22, 3.8, 3.015 * 2.5e-4), rel=1e-6)
+
+
+# ---- variant: geometric extension (App. C) ------------------
+def test_geometric_extension_pins():
+    """e = ||xi + eta|| - ||xi||: (a) hand values on one bond (collinear stretch a -> e = a; transverse b -> e =
+    sqrt(r^2 + b^2) - r while the linearized e is 0); (b) a FINITE rigid rotation leaves every bond length unchanged:
+    e = 0, theta = 0, f = 0 to roundoff, where the linearized model gives a spurious force; (c) e_geo - e_lin is of
+    second order in eta; (d) the App. C pair-scatter code with the extension as printed gives the same force."""
+    r, a, b = 0.5, 1e-3, 2e-3
+    x2 = np.array([[0.0, 0.0, 0.0], [r, 0.0, 0.0]])
+    for u1, e_geo, e_lin in (([a, 0, 0], a, a), ([0, b, 0], np.sqrt(r * r + b * b) - r, 0.0)):
+        u = np.array([[0, 0, 0], u1], float)
+        og = make(x2, 3, MODE_3D, 1.0, extension="geometric", u0=u)
+        ol = make(x2, 3, MODE_3D, 1.0, u0=u)
+        assert og.extension()[0] == pytest.approx(e_geo, rel=1e-12, abs=1e-18)
+        assert ol.extension()[0] == pytest.approx(e_lin, rel=1e-12, abs=1e-18)
+    # (b) finite rotation by 30 degrees about z plus a translation
+    x = lattice((7, 6, 5))
+    c, s_ = np.cos(np.pi / 6), np.sin(np.pi / 6)
+    Rm = np.array([[c, -s_, 0], [s_, c, 0], [0, 0, 1.0]])
+    u = x @ Rm.T - x + np.array([0.3, -0.2, 0.1])
+    og = make(x, 3, MODE_3D, 3.015, extension="geometric", u0=u)
+    ol = make(x, 3, MODE_3D, 3.015, u0=u)
+    fg, fl = og.force_density(), ol.force_density().copy()
+    scale = np.max(np.abs(fl))
+    assert np.max(np.abs(og.e)) <= 1e-13 * 3.0 and np.max(np.abs(og.theta)) <= 1e-12
+    assert np.max(np.abs(fg)) <= 1e-10 * scale and scale > 0
+    # (c) second-order agreement: halving eta quarters the difference
+    rng = np.random.default_rng(3)
+    w = rng.standard_normal(x.shape)
+    d = []
+    for amp in (1e-3, 5e-4):
+        eg = make(x, 3, MODE_3D, 3.015, extension="geometric", u0=amp * w).extension().copy()
+        el = make(x, 3, MODE_3D, 3.015, u0=amp * w).extension().copy()
+        d.append(np.max(np.abs(eg - el)))
+    assert d[0] / d[1] == pytest.approx(4.0, rel=0.02) and d[0] < 1e-4
+    # (d) second formulation: App. C exactly as printed
+    x = lattice((6, 5)) * 1e-3
+    u = 1e-5 * rng.standard_normal(x.shape)
+    vol = np.full(len(x), 1e-9)
+    og = make(x, 2, MODE_PLANE_STRESS, 3.015e-3, vol=vol, extension="geometric", u0=u)
+    f = og.force_density()
+    bonds, Xi, xi = pd_appc.bond_list(x, 3.015e-3)
+    m = pd_appc.weighted_volume(len(x), bonds, xi, vol)
+    PDF, _ = pd_appc.pd_force(u, vol, bonds, m, xi, Xi, np.ones(len(bonds)), og.A, og.K, og.G, geometric=True)
+    assert np.max(np.abs(PDF / vol[:, None] - f)) <= 1e-12 * np.max(np.abs(f))
+
+
+def test_geometric_break_and_run():
+    """the failure stretch of the variant is s = e_geo / xbar; a transverse displacement that stretches the bond past
+    s_c breaks it although the linearized stretch is 0; the stepper conserves momentum like the linearized one"""
+    r, s_c = 1.0, 1e-3
+    b = r * np.sqrt((1 + s_c) ** 2 - 1) * (1 + 1e-9)          # ||xi + eta|| = r (1 + s_c) (1 + ...)
+    x = np.array([[0.0, 0.0], [r, 0.0]])
+    u = np.array([[0.0, 0.0], [0.0, b]])
+    og = make(x, 2, MODE_PLANE_STRAIN, 1.5, s_c=s_c, extension="geometric", u0=u)
+    ol = make(x, 2, MODE_PLANE_STRAIN, 1.5, s_c=s_c, u0=u)
+    assert og.break_bonds()[0] == 2 and ol.break_bonds()[0] == 0
+    x = lattice((9, 7)) * 1e-3
+    rng = np.random.default_rng(5)
+    o = make(x, 2, MODE_PLANE_STRESS, 3.015e-3, vol=np.full(len(x), 1e-9), extension="geometric", dt=5e-8,
+             v0=rng.standard_normal(x.shape))
+    p0 = o.v.sum(0).copy()
+    o.step(50)
+    assert np.allclose(o.v.sum(0), p0, rtol=0, atol=1e-12 * np.abs(o.v).sum())
