@@ -52,6 +52,10 @@ extern "C" {
 #define PD_MODE_PLANE_STRESS 1
 #define PD_MODE_PLANE_STRAIN 2
 
+/* bond extension (pd_material.extension) */
+#define PD_EXT_LINEARIZED 0 /* e = M . (u_j - u_i)  (Eq. 2.7): the model of the paper */
+#define PD_EXT_GEOMETRIC 1  /* e = ||xi + u_j - u_i|| - ||xi||  (App. C listing): variant */
+
 /* per-node boundary flags (pd_boundary.flags) */
 #define PD_CLAMP_X 0x01u /* bits 0-2: dof k clamped: u_k = 0 and v_k = 0 for all time (App. B "FreeDofs", */
 #define PD_CLAMP_Y 0x02u /*           PAPER.md:878); u0/v0 on such dofs are overridden by 0              */
@@ -75,6 +79,9 @@ typedef struct {
   double s_c;       /* critical stretch (Eqs. 1.26/1.28 give it); <= 0 or +inf disables fracture */
   double dt;        /* fixed time increment > 0 (Eq. 2.11)                                      */
   double ramp_time; /* body forces are scaled by g(t_n) = min(1, n*dt/ramp_time); <= 0 => g = 1 */
+  int extension;    /* PD_EXT_LINEARIZED (0, the paper's model and the default) or PD_EXT_GEOMETRIC:
+                       e = ||xi + eta|| - ||xi|| of the paper's loop code (App. C) in
+                       the dilatation, the force and the failure stretch; direction M stays xi/||xi||   */
 } pd_material;
 
 typedef struct {

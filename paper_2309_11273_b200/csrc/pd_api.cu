@@ -174,6 +174,7 @@ int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volum
   if (!(mat->E > 0) || !(mat->nu > -1.0) || !(mat->nu < 0.5) || !(mat->rho > 0) || !(mat->dt > 0) ||
       !(horizon > 0) || !std::isfinite(horizon) || !std::isfinite(mat->E) || !std::isfinite(mat->rho) ||
       !std::isfinite(mat->dt)) { pdi::set_error("E, rho, dt, horizon must be > 0 and nu in (-1, 0.5)"); return PD_ERR_ARG; }
+  if (mat->extension != PD_EXT_LINEARIZED && mat->extension != PD_EXT_GEOMETRIC) { pdi::set_error("unknown extension"); return PD_ERR_ARG; }
   if (bc && bc->n_precut < 0) { pdi::set_error("n_precut < 0"); return PD_ERR_ARG; }
   if (bc && bc->n_precut > 0 && !bc->precut) { pdi::set_error("precut is NULL"); return PD_ERR_ARG; }
   int ndev = 0;
@@ -186,6 +187,7 @@ int pd_create(pd_sim **out, int64_t n, const double *coords, const double *volum
   if (!s) { pdi::set_error("host allocation failed"); return PD_ERR_ALLOC; }
   s->n = n; s->dim = mat->dim; s->mode = mat->mode; s->horizon = horizon;
   s->rho = mat->rho; s->dt = mat->dt; s->ramp_time = mat->ramp_time;
+  s->geom = mat->extension == PD_EXT_GEOMETRIC;
   s->fracture = (mat->s_c > 0.0) && std::isfinite(mat->s_c);
   s->s_c = s->fracture ? mat->s_c : 0.0;
   if (rt && rt->alloc && rt->free) { s->rt = *rt; s->own_alloc = false; }

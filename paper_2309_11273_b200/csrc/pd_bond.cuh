@@ -32,6 +32,28 @@ __device__ __forceinline__ double dot3(const double *x, const double *y) {
   return d;
 }
 
+// GEOM (variant): the geometric extension of the paper's loop code, e = ||xi + eta|| - ||xi||
+// (App. C), in place of the linearized M . eta.  Returned as xbar * e, the quantity the
+// linearized path calls dot = xi . eta, so that everything downstream (theta, break test, e / xbar = dot / ||xi||^2)
+// is unchanged.  Evaluated like the listing (and the oracle): squares summed in component order, individually
+// rounded, two square roots.
+template <int DIM>
+__device__ __forceinline__ double dot_geom(const double *xi, const double *eta) {
+  double r2 = __dmul_rn(xi[0], xi[0]), y2;
+  {
+    const double y = __dadd_rn(xi[0], eta[0]);
+    y2 = __dmul_rn(y, y);
+  }
+#pragma unroll
+  for (int k = 1; k < DIM; ++k) {
+    const double y = __dadd_rn(xi[k], eta[k]);
+    r2 = __dadd_rn(r2, __dmul_rn(xi[k], xi[k]));
+    y2 = __dadd_rn(y2, __dmul_rn(y, y));
+  }
+  const double xbar = sqrt(r2);
+  return __dmul_rn(xbar, __dsub_rn(sqrt(y2), xbar));
+}
+
 // dilatation (+ break) policy: R rows per lane.
 // FILT (lattice layout): the fast pass does not evaluate dot - s_c ||xi||^2 per bond; it keeps the
 // maximum of the HIGH WORDS of dot over a step and compares it with the high word of
@@ -39,7 +61,7 @@ __device__ __forceinline__ double dot3(const double *x, const double *y) {
 // hi(dot) < hi(thr) => dot < thr <= s_c ||xi||^2 => the exact test is negative.  Anything else sends
 // the bonds to the masked variant, which evaluates the exact test.  (Integer compares on the ALU pipe
 // instead of 4 FP64 instructions per bond.)
-template <int DIM, bool FRAC, bool UNIV, int R, bool FILT = false>
+template <int DIM, bool FRAC, bool UNIV, int R, bool FILT = false, bool GEOM = false>
 struct DilPolicy {
   using E = Ent<DIM, false, !UNIV>;
   static constexpr bool kFrac = FRAC;
@@ -81,7 +103,7 @@ struct DilPolicy {
       xi[k] = e.p[k].x - xo[r][k];
       eta[k] = e.p[k].y - uo[r][k];
     }
-    const double dot = dot3<DIM>(xi, eta);
+    const double dot = GEOM ? dot_geom<DIM>(xi, eta) : dot3<DIM>(xi, eta);
     bool brk = false;
     if (!MASKED) in = true;
     if (FRAC && FILT && !MASKED) {
@@ -116,7 +138,7 @@ struct DilPolicy {
   // in / nofail: bit r = row r (MASKED only); returns the rows whose bond breaks now
   template <bool MASKED>
   __device__ __forceinline__ uint32_t finish(uint32_t in, uint32_t nofail) {
-    static_assert(UNIV, "staged form: uniform volume only");
+    static_assert(UNIV, "staged form: uniform volume only");   // (never taken with GEOM: the lattice kernels launch GEOM unstaged)
     double dot[R], r2[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) dot[r] = __dmul_rn(xi_[r][0], eta_[r][0]);
@@ -168,7 +190,7 @@ __device__ __forceinline__ double rcp_seed(double x) {
 }
 
 // force policy
-template <int DIM, bool UNIV, int R>
+template <int DIM, bool UNIV, int R, bool GEOM = false>
 struct ForcePolicy {
   using E = Ent<DIM, true, !UNIV>;
   static constexpr bool kFrac = false;
@@ -185,7 +207,7 @@ struct ForcePolicy {
       xi[k] = e.p[k].x - xo[r][k];
       eta[k] = e.p[k].y - uo[r][k];
     }
-    const double dot = dot3<DIM>(xi, eta);
+    const double dot = GEOM ? dot_geom<DIM>(xi, eta) : dot3<DIM>(xi, eta);
     const double r2 = dot3<DIM>(xi, xi);
     // d = dot / r2 = e / xbar: seed y, err = 1 - r2 y, d = dot y (1 + err + err^2)  (relative error err^3 ~ 2^-60)
     const double y = rcp_seed(r2);
@@ -215,7 +237,7 @@ struct ForcePolicy {
   }
   template <bool MASKED>
   __device__ __forceinline__ uint32_t finish(uint32_t in, uint32_t) {
-    static_assert(UNIV, "staged form: uniform volume only");
+    static_assert(UNIV, "staged form: uniform volume only");   // (never taken with GEOM: the lattice kernels launch GEOM unstaged)
     double dot[R], r2[R], y[R], err[R], q[R], t[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) r2[r] = __dmul_rn(xi_[r][0], xi_[r][0]);

@@ -149,6 +149,7 @@ struct pd_sim {
   double horizon = 0, A = 0, K = 0, G = 0, c1 = 0;  // c1 = K - G/3
   double rho = 0, dt = 0, s_c = 0, ramp_time = 0, vol_uniform = 0;
   bool fracture = false, uniform_v = false, has_nofail = false, has_bc = false;
+  bool geom = false;            // variant: geometric extension e = ||xi + eta|| - ||xi|| (App. C) instead of the linearized one
   int kdiv = 1;
   // runtime
   pd_runtime rt{};

@@ -492,7 +492,7 @@ int build_lattice(pd_sim *s, const PdGrid &g, const double *coords, const double
     l.wbeg[w] = c;
   }
   l.uniform = false;
-  bool want_uniform = true;
+  bool want_uniform = !s->geom;   // (the geometric-extension variant needs xi + eta per bond)
   if (const char *env = getenv("PD_LAT_UNIFORM")) want_uniform = atoi(env) != 0;
   if (want_uniform) {
     bool ok = true;

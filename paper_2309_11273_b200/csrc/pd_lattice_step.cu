@@ -27,8 +27,8 @@ using pdb::FULL;
 constexpr int TPB = 256;
 inline unsigned nblk(int64_t n) { return (unsigned)((n + TPB - 1) / TPB); }
 
-template <int DIM, bool FORCE, bool FRAC, int R> struct PolicyOfR { using type = pdb::DilPolicy<DIM, FRAC, true, R, true>; };
-template <int DIM, bool FRAC, int R> struct PolicyOfR<DIM, true, FRAC, R> { using type = pdb::ForcePolicy<DIM, true, R>; };
+template <int DIM, bool FORCE, bool FRAC, int R, bool GEOM> struct PolicyOfR { using type = pdb::DilPolicy<DIM, FRAC, true, R, true, GEOM>; };
+template <int DIM, bool FRAC, int R, bool GEOM> struct PolicyOfR<DIM, true, FRAC, R, GEOM> { using type = pdb::ForcePolicy<DIM, true, R, GEOM>; };
 
 }  // namespace
 
@@ -137,11 +137,11 @@ struct DirArgs {
   struct Col { int off; uint8_t n, word, bit0, pad; } cols[PD_LAT_MAXCOL];   // off = (dz*DY + dy0)*DX + dx (dense cells)
 };
 
-template <int DIM, bool FORCE, bool FRAC, int MAXT, int MINB, bool STAGED, int R>
+template <int DIM, bool FORCE, bool FRAC, int MAXT, int MINB, bool STAGED, int R, bool GEOM = false>
 __global__ void __launch_bounds__(MAXT, MINB) k_lat_direct(const __grid_constant__ DirArgs a) {
   extern __shared__ __align__(16) unsigned char smraw[];
   constexpr int NPAIR = FORCE ? DIM + 1 : DIM;
-  using P = typename PolicyOfR<DIM, FORCE, FRAC, R>::type;
+  using P = typename PolicyOfR<DIM, FORCE, FRAC, R, GEOM>::type;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
   // shared: column table, thresholds, per-warp mask words [nwarp][4 words][4 rows][32]
   DirArgs::Col *scol = (DirArgs::Col *)smraw;
@@ -337,6 +337,7 @@ DirPrepared *dir_prepare(pd_sim *s, bool force) {
   a.DX = l.DX; a.DY = l.DY; a.HX = l.HX; a.HY = l.HY; a.HZ = l.HZ; a.PZ = l.PZ;
   a.rows = env_int(force ? "PD_DIR_FRC_ROWS" : "PD_DIR_DIL_ROWS", s->dim == 2 ? 2 : 4);   // rows per lane
   if (a.rows != 2 && !(a.rows == 1 && s->dim == 2)) a.rows = 4;
+  if (s->geom) a.rows = 2;
   a.nxc = l.PX / 32; a.nyq = (l.PY + 8) / 4; a.nyq_used = l.PY / a.rows;
   a.ncol = l.ncol; a.nw = l.nw;
   a.cy = std::max(1, std::min(env_int(force ? "PD_DIR_FRC_CY" : "PD_DIR_DIL_CY", 2), 4));
@@ -392,7 +393,9 @@ int dir_launch(pd_sim *s, bool force, double *theta_out, bool frac) {
   static const int staged = env_int("PD_DIR_STAGED", 2);   // bit 0: dilatation, bit 1: force (phase-ordered step, pd_bond.cuh)
 #define DIR_LAUNCH(DIM_, FORCE_, FRAC_, MINB_, ST_)                                                                        \
   do {                                                                                                                     \
-    if (a.rows == 1 && DIM_ == 2) k_lat_direct<2, FORCE_, FRAC_, 128, 4, false, 1><<<pp->grid, pp->block, pp->smem, s->stream>>>(a); \
+    if (s->geom) /* geometric extension (variant): 2 rows per lane (dir_prepare), bond by bond */                          \
+      k_lat_direct<DIM_, FORCE_, FRAC_, 128, 2, false, 2, true><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);          \
+    else if (a.rows == 1 && DIM_ == 2) k_lat_direct<2, FORCE_, FRAC_, 128, 4, false, 1><<<pp->grid, pp->block, pp->smem, s->stream>>>(a); \
     else if (a.rows == 2) k_lat_direct<DIM_, FORCE_, FRAC_, 128, (FORCE_ ? 3 : 4), false, 2><<<pp->grid, pp->block, pp->smem, s->stream>>>(a); \
     else if (ST_) k_lat_direct<DIM_, FORCE_, FRAC_, 128, MINB_, true, 4><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);  \
     else k_lat_direct<DIM_, FORCE_, FRAC_, 128, MINB_, false, 4><<<pp->grid, pp->block, pp->smem, s->stream>>>(a);          \

@@ -194,13 +194,13 @@ __device__ __forceinline__ void walk_group(P &p, const StepArgs &a, int64_t grp,
 }
 
 // ---------------------------------------------------------------------------------------------
-template <int DIM, bool FRAC, bool UNIV>
+template <int DIM, bool FRAC, bool UNIV, bool GEOM>
 __global__ void __launch_bounds__(TPB, 3) k_dilatation(StepArgs a) {
   const int lane = threadIdx.x & 31;
   const int64_t grp = ((int64_t)blockIdx.x * TPB + threadIdx.x) >> 5;
   if (grp >= a.ngroups) return;
   const uint32_t e0 = pd_elem(grp * PD_R * 32 + lane);
-  pdb::DilPolicy<DIM, FRAC, UNIV, PD_R> p;
+  pdb::DilPolicy<DIM, FRAC, UNIV, PD_R, false, GEOM> p;
   p.s_c = a.s_c;
 #pragma unroll
   for (int r = 0; r < PD_R; ++r) {
@@ -226,13 +226,13 @@ __global__ void __launch_bounds__(TPB, 3) k_dilatation(StepArgs a) {
 }
 
 // ---------------------------------------------------------------------------------------------
-template <int DIM, bool UNIV>
+template <int DIM, bool UNIV, bool GEOM>
 __global__ void __launch_bounds__(TPB, 2) k_force_update(StepArgs a) {
   const int lane = threadIdx.x & 31;
   const int64_t grp = ((int64_t)blockIdx.x * TPB + threadIdx.x) >> 5;
   if (grp >= a.ngroups) return;
   const uint32_t e0 = pd_elem(grp * PD_R * 32 + lane);
-  pdb::ForcePolicy<DIM, UNIV, PD_R> p;
+  pdb::ForcePolicy<DIM, UNIV, PD_R, GEOM> p;
 #pragma unroll
   for (int r = 0; r < PD_R; ++r) {
     const uint32_t e = e0 + r * 32 * PD_NP;
@@ -358,14 +358,14 @@ StepArgs make_args(pd_sim *s) {
 
 inline unsigned ngrid(const pd_sim *s) { return (unsigned)((s->ngroups + PD_GROUPS_PER_CTA - 1) / PD_GROUPS_PER_CTA); }
 
-template <int DIM>
+template <int DIM, bool GEOM>
 void dil_dispatch(const StepArgs &a, bool frac, bool univ, unsigned grid, cudaStream_t st) {
-  if (frac) { if (univ) k_dilatation<DIM, true, true><<<grid, TPB, 0, st>>>(a); else k_dilatation<DIM, true, false><<<grid, TPB, 0, st>>>(a); }
-  else { if (univ) k_dilatation<DIM, false, true><<<grid, TPB, 0, st>>>(a); else k_dilatation<DIM, false, false><<<grid, TPB, 0, st>>>(a); }
+  if (frac) { if (univ) k_dilatation<DIM, true, true, GEOM><<<grid, TPB, 0, st>>>(a); else k_dilatation<DIM, true, false, GEOM><<<grid, TPB, 0, st>>>(a); }
+  else { if (univ) k_dilatation<DIM, false, true, GEOM><<<grid, TPB, 0, st>>>(a); else k_dilatation<DIM, false, false, GEOM><<<grid, TPB, 0, st>>>(a); }
 }
-template <int DIM>
+template <int DIM, bool GEOM>
 void force_dispatch(const StepArgs &a, bool univ, unsigned grid, cudaStream_t st) {
-  if (univ) k_force_update<DIM, true><<<grid, TPB, 0, st>>>(a); else k_force_update<DIM, false><<<grid, TPB, 0, st>>>(a);
+  if (univ) k_force_update<DIM, true, GEOM><<<grid, TPB, 0, st>>>(a); else k_force_update<DIM, false, GEOM><<<grid, TPB, 0, st>>>(a);
 }
 
 }  // namespace
@@ -377,8 +377,13 @@ int launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
   StepArgs a = make_args(s);
   a.theta_out = theta_out;
   const bool frac = do_break && s->fracture;
-  if (s->dim == 2) dil_dispatch<2>(a, frac, s->uniform_v, ngrid(s), s->stream);
-  else dil_dispatch<3>(a, frac, s->uniform_v, ngrid(s), s->stream);
+  if (s->geom) {
+    if (s->dim == 2) dil_dispatch<2, true>(a, frac, s->uniform_v, ngrid(s), s->stream);
+    else dil_dispatch<3, true>(a, frac, s->uniform_v, ngrid(s), s->stream);
+  } else {
+    if (s->dim == 2) dil_dispatch<2, false>(a, frac, s->uniform_v, ngrid(s), s->stream);
+    else dil_dispatch<3, false>(a, frac, s->uniform_v, ngrid(s), s->stream);
+  }
   return PD_OK;
 }
 
@@ -386,8 +391,13 @@ int launch_force_update(pd_sim *s) {
   if (s->lat.on) return lat_launch_force_update(s);
   StepArgs a = make_args(s);
   a.nbw = s->nb[s->cur ^ 1];
-  if (s->dim == 2) force_dispatch<2>(a, s->uniform_v, ngrid(s), s->stream);
-  else force_dispatch<3>(a, s->uniform_v, ngrid(s), s->stream);
+  if (s->geom) {
+    if (s->dim == 2) force_dispatch<2, true>(a, s->uniform_v, ngrid(s), s->stream);
+    else force_dispatch<3, true>(a, s->uniform_v, ngrid(s), s->stream);
+  } else {
+    if (s->dim == 2) force_dispatch<2, false>(a, s->uniform_v, ngrid(s), s->stream);
+    else force_dispatch<3, false>(a, s->uniform_v, ngrid(s), s->stream);
+  }
   return PD_OK;
 }
 

@@ -22,7 +22,7 @@ EXPORTS = ["pd_create", "pd_step", "pd_get_u", "pd_get_v", "pd_get_damage", "pd_
 
 class PdMaterial(C.Structure):
     _fields_ = [("dim", C.c_int), ("mode", C.c_int), ("E", C.c_double), ("nu", C.c_double), ("rho", C.c_double),
-                ("s_c", C.c_double), ("dt", C.c_double), ("ramp_time", C.c_double)]
+                ("s_c", C.c_double), ("dt", C.c_double), ("ramp_time", C.c_double), ("extension", C.c_int)]
 
 
 class PdBoundary(C.Structure):
@@ -116,7 +116,8 @@ class Sim:
     """One simulation handle (pd_sim*)."""
 
     def __init__(self, coords, volumes, horizon, *, dim, mode, E, nu, rho, dt, s_c=0.0, ramp_time=0.0, flags=None,
-                 value=None, precut=None, u0=None, v0=None, device="cuda:0", use_torch_allocator=True):
+                 value=None, precut=None, u0=None, v0=None, device="cuda:0", use_torch_allocator=True,
+                 extension="linearized"):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: paper_2309_11273_b200 has no CPU path")
@@ -149,7 +150,7 @@ class Sim:
         v0 = prep(v0, np.float64)
         precut = prep(precut, np.int32)
         npre = 0 if precut is None else int(np.prod(precut.shape)) // 2
-        mat = PdMaterial(dim, mode, E, nu, rho, s_c, dt, ramp_time)
+        mat = PdMaterial(dim, mode, E, nu, rho, s_c, dt, ramp_time, {"linearized": 0, "geometric": 1}[extension])
         bc = PdBoundary(_ptr(flags), _ptr(value), _ptr(precut) if npre else None, npre, _ptr(u0), _ptr(v0))
         self._rt = _TorchRuntime(self.device) if use_torch_allocator else None
         h = C.c_void_p()

@@ -288,3 +288,47 @@ def test_full_size_config5p_sampled():
     idx = rng.integers(0, wl.n, 2000)
     assert np.allclose(sim.get_damage()[idx], o.damage()[idx], rtol=0, atol=1e-12)
     sim.destroy()
+
+
+@pytest.mark.parametrize("generic", [False, True])
+def test_geometric_extension_variant(generic, monkeypatch):
+    """the geometric extension e = ||xi + eta|| - ||xi|| of App. C in the dilatation,
+    the force and the failure stretch (pd_material.extension = PD_EXT_GEOMETRIC), against the oracle's variant:
+    a FINITE rigid rotation gives zero force, trajectories agree to 1e-10, broken sets are identical."""
+    from paper_2309_11273_b200 import pd, workloads as W
+    from oracle.pd_oracle import PDOracle
+    for k in _ENV_KEYS:
+        monkeypatch.delenv(k, raising=False)
+    if generic:
+        monkeypatch.setenv("PD_FORCE_GENERIC", "1")
+    # finite rotation: zero force with the geometric extension (the linearized model pushes back)
+    wl = W.block3d(nx=16, ny=9, nz=8)
+    x = wl.coords
+    c, s_ = np.cos(0.4), np.sin(0.4)
+    u0 = x @ np.array([[c, -s_, 0], [s_, c, 0], [0, 0, 1.0]]).T - x
+    kw = dict(wl.material_kwargs()); kw["dt"] = 1e-7
+    sim = pd.Sim(x, wl.volumes, wl.horizon, **kw, u0=u0, extension="geometric")
+    assert sim.get_layout()["layout"] == (0 if generic else 1)
+    sim.step(1)
+    v_geo = np.abs(sim.get_v()).max()
+    sim.destroy()
+    sim = pd.Sim(x, wl.volumes, wl.horizon, **kw, u0=u0)
+    sim.step(1)
+    v_lin = np.abs(sim.get_v()).max()
+    sim.destroy()
+    assert v_geo <= 1e-9 * v_lin and v_lin > 0
+    # trajectories and broken sets
+    for wl, nsteps in ((W.block3d(nx=21, ny=10, nz=9), 60), (W.branching2d(nx=80, ny=40, steps=500), 420),
+                       (W.cylinder3d(r_cells=8, l_cells=30, omega=400.0), 120)):
+        o = PDOracle(wl.coords, wl.volumes, wl.horizon, **wl.material_kwargs(), flags=wl.flags, value=wl.value,
+                     precut=wl.precut, u0=wl.u0, v0=wl.v0, extension="geometric")
+        sim = pd.Sim.from_workload(wl, extension="geometric")
+        assert sim.get_layout()["layout"] == (0 if generic else 1)   # the uniform-lattice path is linearized only
+        sim.step(nsteps); o.step(nsteps)
+        assert _rel(sim.get_u(), o.u) <= (TOL if wl.s_c == 0 else 1e-9), wl.name
+        assert _rel(sim.get_v(), o.v) <= (TOL if wl.s_c == 0 else 1e-9), wl.name
+        bs, _, _ = _broken_set(sim)
+        assert bs == o.broken_set() and o.near_total == 0, wl.name
+        if wl.s_c > 0:
+            assert len(bs) > 2 * len(wl.precut), "the case must actually break bonds"
+        sim.destroy()
