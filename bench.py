@@ -318,6 +318,45 @@ def measure(name, K, Wm, local, world, want_e2e, want_cpu):
     return line
 
 
+def measure_matrix(name, K, Wm, local):
+    """the paper's own 4-SpMV scheme (pd_matrix_*, App. B) on this GPU, on the workload with fracture switched off
+    (App. B has no failure step), beside the matrix-free path on the same input: the on-box comparison of DESIGN.md 6"""
+    import dataclasses
+    import torch
+    from paper_2309_11273_b200 import pd
+    wl = dataclasses.replace(make_workload(name), s_c=0.0, precut=np.zeros((0, 2), np.int32))
+    K = K or 100
+    res = {}
+    sim = pd.Sim.from_workload(wl, device=f"cuda:{local}")
+    n, z = sim.n, sim.get_layout()["n_directed_bonds"]
+    t0 = time.perf_counter()
+    ms_ = pd.MatrixScheme.from_workload(sim, wl)
+    torch.cuda.synchronize()
+    t_asm = time.perf_counter() - t0
+    for label, obj in (("matrix_free", sim), ("matrix_scheme", ms_)):
+        obj.step(Wm)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); obj.step(K); e1.record(); torch.cuda.synchronize()
+        res[label] = e0.elapsed_time(e1) / K
+    u, v, info = ms_.get()
+    err = float(np.linalg.norm(u - sim.get_u()) / max(np.linalg.norm(u), 1e-300))
+    ms_.destroy(); sim.destroy()
+    # bytes the scheme streams per step: every matrix entry (8 B value + 4 B column) once, the row pointers, the vectors
+    nnz = info["nnz_CE"] + info["nnz_CTH"] + info["nnz_KTH"] + info["nnz_KE"]
+    vec = 8 * (2 * info["n_bonds"] * 2 + n * (1 + 7 * wl.dim))
+    bytes_step = info["matrix_bytes"] + vec
+    t = res["matrix_scheme"] * 1e-3
+    return {"scheme": "matrix (App. B: 4 CSR SpMV + update, hand-written FP64 kernels)", "metric": METRIC, "unit": "node-steps/s",
+            "value": n / t, "ms_per_step": res["matrix_scheme"], "steps": K, "warmup": Wm, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{name}:{wl.name} (fracture off)", "nodes": n, "directed_bonds": z, "undirected_bonds": info["n_bonds"],
+                       "nnz": {k: info[k] for k in ("nnz_CE", "nnz_CTH", "nnz_KTH", "nnz_KE")}, "matrix_bytes": info["matrix_bytes"],
+                       "assembly_seconds": t_asm},
+            "bytes_per_step": bytes_step, "bytes_per_directed_bond_step": bytes_step / z, "achieved_GBps": bytes_step / t / 1e9,
+            "matrix_free_ms_per_step": res["matrix_free"], "speedup_matrix_free_over_matrix": res["matrix_scheme"] / res["matrix_free"],
+            "relL2_u_matrix_vs_matrix_free": err}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -326,6 +365,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config5")
     ap.add_argument("--out", default=None, help="--workload all: write the per-config records to this JSON file")
+    ap.add_argument("--scheme", default="matrix-free", choices=["matrix-free", "matrix"],
+                    help="matrix: time the paper's own 4-SpMV scheme on this GPU beside the matrix-free path (fracture off)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -343,6 +384,12 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     Wm = max(args.warmup, 3)
 
+    if args.scheme == "matrix":
+        if rank == 0:
+            print(json.dumps(measure_matrix("config4" if args.workload == "all" else args.workload, args.steps, Wm, local)))
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
     if args.workload == "all":
         recs = []
         for name in ALL:

@@ -178,6 +178,24 @@ PD_API int pd_get_layout(pd_sim *sim, int64_t counts[8]);
  * ms[0] = dilatation(+break) kernel, ms[1] = force+update kernel.  Synchronises. */
 PD_API int pd_step_timed(pd_sim *sim, int64_t nsteps, double ms[2]);
 
+/* ---- the paper's own scheme, as an on-box comparison for the matrix-free path ----
+ * pd_matrix_create assembles, on the device, the four global sparse matrices CE (Nb x d n), CTH (n x Nb), KTH (d n x n),
+ * KE (d n x Nb) of Eqs. 2.7-2.10 in CSR (int64 row pointers, int32 columns, FP64 values), user
+ * node order, from the family of an existing handle:
+ *   rowptr[n+1], col[Z]  the directed family as returned by pd_get_bond_mask; m[n] as returned by pd_get_node_fields
+ *   coords, volumes, material, boundary  as for pd_create (pre-cuts and s_c are ignored: App. B has no failure step)
+ *   stream  cudaStream_t or NULL.  All pointers host or device; inputs are copied.
+ * pd_matrix_step runs the solver body of App. B: E = CE U; Theta = CTH E; PDF = KTH Theta + KE E;
+ * RF = EXF + PDF; ACC = RF./M; VEL += ACC Dt; U(FreeDofs) += Dt VEL(FreeDofs) -- 4 hand-written CSR SpMVs + 1 vector
+ * kernel per step, asynchronous.  pd_matrix_get copies U and VEL (dim*n each, may be NULL) and fills
+ * info = {n, Nb, nnz(CE), nnz(CTH), nnz(KTH), nnz(KE), bytes of the four matrices, step}; synchronises. */
+typedef struct pd_matrix pd_matrix;
+PD_API int pd_matrix_create(pd_matrix **out, int64_t n, const double *coords, const double *volumes, const pd_material *material,
+                            const pd_boundary *boundary, const int64_t *rowptr, const int32_t *col, const double *m, void *stream);
+PD_API int pd_matrix_step(pd_matrix *pm, int64_t nsteps);
+PD_API int pd_matrix_get(pd_matrix *pm, double *u, double *v, int64_t info[8]);
+PD_API int pd_matrix_destroy(pd_matrix *pm);
+
 PD_API const char *pd_last_error(void);
 PD_API const char *pd_version(void);
 

@@ -17,7 +17,8 @@ _LIBPATH = os.environ.get("PD_LIBPATH") or os.path.join(_HERE, "libpd.so")   # P
 
 PD_OK, PD_ERR_ARG, PD_ERR_ISOLATED, PD_ERR_ALLOC, PD_ERR_CUDA, PD_ERR_LIMIT = 0, -1, -2, -3, -4, -5
 EXPORTS = ["pd_create", "pd_step", "pd_get_u", "pd_get_v", "pd_get_damage", "pd_destroy", "pd_get_stats",
-           "pd_get_bond_mask", "pd_get_node_fields", "pd_get_layout", "pd_step_timed", "pd_last_error", "pd_version"]
+           "pd_get_bond_mask", "pd_get_node_fields", "pd_get_layout", "pd_step_timed", "pd_last_error", "pd_version",
+           "pd_matrix_create", "pd_matrix_step", "pd_matrix_get", "pd_matrix_destroy"]
 
 
 class PdMaterial(C.Structure):
@@ -70,6 +71,11 @@ def load():
         lib.pd_get_node_fields.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         lib.pd_get_layout.argtypes = [C.c_void_p, C.c_void_p]
         lib.pd_step_timed.argtypes = [C.c_void_p, C.c_int64, C.c_void_p]
+        lib.pd_matrix_create.argtypes = [C.POINTER(C.c_void_p), C.c_int64, C.c_void_p, C.c_void_p, C.POINTER(PdMaterial),
+                                         C.POINTER(PdBoundary), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.pd_matrix_step.argtypes = [C.c_void_p, C.c_int64]
+        lib.pd_matrix_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.pd_matrix_destroy.argtypes = [C.c_void_p]
         _lib = lib
     return _lib
 
@@ -243,6 +249,60 @@ class Sim:
     def destroy(self):
         if getattr(self, "h", None):
             self.lib.pd_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+class MatrixScheme:
+    """The paper's own 4-SpMV scheme (pd_matrix_* of include/pd.h) on the family of an existing Sim: the on-box
+    comparison for the matrix-free path (no fracture).  Argument marshalling only."""
+
+    def __init__(self, sim, coords, volumes, *, dim, mode, E, nu, rho, dt, s_c=0.0, ramp_time=0.0, flags=None, value=None,
+                 u0=None, v0=None, **_ignored):
+        import torch
+        self.lib, self.n, self.dim = sim.lib, sim.n, int(dim)
+        rowptr, col, _ = sim.get_bond_mask()
+        m, _ = sim.get_node_fields(want_theta=False)
+        keep = [np.ascontiguousarray(coords, np.float64), np.ascontiguousarray(volumes, np.float64), rowptr, col, m]
+        opt = [None if a is None else np.ascontiguousarray(a, dt_) for a, dt_ in
+               ((flags, np.uint8), (value, np.float64), (u0, np.float64), (v0, np.float64))]
+        mat = PdMaterial(dim, mode, E, nu, rho, 0.0, dt, ramp_time, 0)
+        bc = PdBoundary(_ptr(opt[0]), _ptr(opt[1]), None, 0, _ptr(opt[2]), _ptr(opt[3]))
+        h = C.c_void_p()
+        stream = C.c_void_p(torch.cuda.current_stream(sim.device).cuda_stream)
+        rc = self.lib.pd_matrix_create(C.byref(h), self.n, _ptr(keep[0]), _ptr(keep[1]), C.byref(mat), C.byref(bc),
+                                       _ptr(rowptr), _ptr(col), _ptr(m), stream)
+        if rc != PD_OK:
+            raise PdError(rc, self.lib.pd_last_error().decode())
+        self.h = h
+
+    @classmethod
+    def from_workload(cls, sim, wl):
+        return cls(sim, wl.coords, wl.volumes, **wl.material_kwargs(), flags=wl.flags, value=wl.value, u0=wl.u0, v0=wl.v0)
+
+    def step(self, nsteps=1):
+        rc = self.lib.pd_matrix_step(self.h, int(nsteps))
+        if rc != PD_OK:
+            raise PdError(rc, self.lib.pd_last_error().decode())
+
+    def get(self):
+        """(u, v, info) with info = dict(n, n_bonds, nnz_CE, nnz_CTH, nnz_KTH, nnz_KE, matrix_bytes, step)"""
+        u, v = np.empty((self.n, self.dim)), np.empty((self.n, self.dim))
+        info = (C.c_int64 * 8)()
+        rc = self.lib.pd_matrix_get(self.h, _ptr(u), _ptr(v), C.addressof(info))
+        if rc != PD_OK:
+            raise PdError(rc, self.lib.pd_last_error().decode())
+        keys = ["n", "n_bonds", "nnz_CE", "nnz_CTH", "nnz_KTH", "nnz_KE", "matrix_bytes", "step"]
+        return u, v, dict(zip(keys, [int(x) for x in info]))
+
+    def destroy(self):
+        if getattr(self, "h", None):
+            self.lib.pd_matrix_destroy(self.h)
             self.h = None
 
     def __del__(self):

@@ -332,3 +332,20 @@ def test_geometric_extension_variant(generic, monkeypatch):
         if wl.s_c > 0:
             assert len(bs) > 2 * len(wl.precut), "the case must actually break bonds"
         sim.destroy()
+
+
+def test_matrix_scheme_matches_oracle():
+    """the paper's matrix-based scheme (CE, CTH, KTH, KE of Eqs. 2.7-2.10 + the solver body of App. B,
+    PAPER.md:860-885) with hand-written CSR SpMVs, against the oracle (no fracture): relative L2 of u, v <= 1e-10,
+    and against the matrix-free path of the same library"""
+    from paper_2309_11273_b200 import pd, workloads as W
+    for wl, nsteps in ((W.cantilever2d(), 300), (W.block3d(nx=24, ny=11, nz=9), 80)):
+        sim, o = _sim(wl), _oracle(wl)
+        ms = pd.MatrixScheme.from_workload(sim, wl)
+        ms.step(nsteps); sim.step(nsteps); o.step(nsteps)
+        u, v, info = ms.get()
+        assert info["n_bonds"] * 2 == o.Z and info["nnz_CE"] == 2 * wl.dim * info["n_bonds"] and info["step"] == nsteps
+        assert info["nnz_KTH"] == wl.dim * (o.Z + wl.n) and info["nnz_KE"] == wl.dim * o.Z and info["nnz_CTH"] == o.Z
+        assert _rel(u, o.u) <= TOL and _rel(v, o.v) <= TOL, wl.name
+        assert _rel(u, sim.get_u()) <= TOL
+        ms.destroy(); sim.destroy()
