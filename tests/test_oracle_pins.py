@@ -457,3 +457,64 @@ def test_geometric_break_and_run():
     p0 = o.v.sum(0).copy()
     o.step(50)
     assert np.allclose(o.v.sum(0), p0, rtol=0, atol=1e-12 * np.abs(o.v).sum())
+
+
+# ---- NEXT row f1: adaptive dynamic relaxation --------------------------
+def test_adr_converges_to_direct_solve():
+    """ADR on the oracle's force: (a) 1-dof spring analogue (two nodes, one clamped) -> U = F/k; (b) zero load -> 0;
+    (c) a small 3-D bar, one end clamped, body force on the other end layer AND a prescribed-displacement variant:
+    the converged U equals the direct dense solve of K U = F (K assembled from the linear oracle force) to 1e-6."""
+    from oracle.pd_adr import ADROracle, dense_stiffness
+    # (a) two nodes on the x axis, node 0 clamped, body force b on node 1 (x only; y clamped on both)
+    x = np.array([[0.0, 0.0], [1.0, 0.0]])
+    fl = np.array([3, 2 | 64], np.uint8)
+    val = np.array([[0.0, 0.0], [2.5, 0.0]])
+    o = make(x, 2, MODE_PLANE_STRAIN, 1.5, E=3.0, nu=0.25, flags=fl, value=val)
+    K = dense_stiffness(o)
+    k = K[2, 2]
+    adr = ADROracle(o, lam=0.3 * k)
+    adr.iterate(400)
+    assert o.u[1, 0] == pytest.approx(2.5 / k, rel=1e-8) and np.all(o.u[0] == 0)
+    # (b) zero load
+    o = make(x, 2, MODE_PLANE_STRAIN, 1.5, E=3.0, nu=0.25, flags=np.array([3, 2], np.uint8))
+    ADROracle(o, lam=1.0).iterate(5)
+    assert np.all(o.u == 0.0)
+    # (c) bar 10 x 4 x 4, clamp x < 2 cells
+    xb = lattice((10, 4, 4))
+    ix = xb[:, 0]
+    fl = np.zeros(len(xb), np.uint8)
+    fl[ix < 2] = 7
+    val = np.zeros_like(xb)
+    for mode in ("force", "displacement"):
+        f2, v2 = fl.copy(), val.copy()
+        if mode == "force":
+            f2[ix > 8.5] |= 64
+            v2[ix > 8.5] = [1e-3, 2e-4, 0.0]
+        o = make(xb, 3, MODE_3D, 2.015, E=1.0, nu=0.25, flags=f2, value=v2)
+        K = dense_stiffness(o)
+        assert np.max(np.abs(K - K.T)) <= 1e-12 * np.max(np.abs(K))
+        lam = 1.05 * 0.25 * np.linalg.eigvalsh(K)[-1]
+        fixed = np.repeat(f2 & 7, 3).reshape(-1, 3)
+        fixed = np.stack([(f2 & (1 << k_)) != 0 for k_ in range(3)], axis=1).reshape(-1)
+        rhs = np.where(((f2 & 64) != 0)[:, None], v2, 0.0).reshape(-1)
+        uc = np.zeros(len(rhs))
+        if mode == "displacement":        # drive the end layer to u_x = 1e-3 in 50 increments, then relax
+            f2[ix > 8.5] |= 8
+            v2[ix > 8.5] = [2e-5, 0.0, 0.0]
+            o = make(xb, 3, MODE_3D, 2.015, E=1.0, nu=0.25, flags=f2, value=v2)
+            adr = ADROracle(o, lam)
+            adr.iterate(50)
+            o.value[:] = 0.0              # hold
+            adr.iterate(3000)
+            drv = np.stack([(f2 & (8 << k_)) != 0 for k_ in range(3)], axis=1).reshape(-1)
+            uc[drv] = 50 * 2e-5
+            fixed = fixed | drv
+        else:
+            adr = ADROracle(o, lam)
+            adr.iterate(3000)
+        free = ~fixed
+        usol = uc.copy()
+        usol[free] = np.linalg.solve(K[np.ix_(free, free)], rhs[free] - K[np.ix_(free, fixed)] @ uc[fixed])
+        err = np.linalg.norm(o.u.reshape(-1) - usol) / np.linalg.norm(usol)
+        assert err <= 1e-6, (mode, err)
+        assert max(adr.c_hist) > 0.0      # the adaptive damping was active
