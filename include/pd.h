@@ -178,6 +178,18 @@ PD_API int pd_get_layout(pd_sim *sim, int64_t counts[8]);
  * ms[0] = dilatation(+break) kernel, ms[1] = force+update kernel.  Synchronises. */
 PD_API int pd_step_timed(pd_sim *sim, int64_t nsteps, double ms[2]);
 
+/* ---- quasi-static driver: adaptive dynamic relaxation ----
+ * The paper solves its Ex. 4 "by using an adaptive dynamic relaxation algorithm presented in [Underwood 1983; Kilic &
+ * Madenci 2010]" and does not restate it; this is that algorithm with a uniform fictitious density
+ * Lambda = lam I and pseudo time step 1, on top of the dilatation / force kernels of pd_step:
+ *   R^n = f(U^n) + g b;  1K_ii = -(R_i^n - R_i^{n-1}) / (lam Ud_i^{n-1/2});  c^n = 2 sqrt((U.1K U)/(U.U)) over the free dofs
+ *   Ud^{n+1/2} = ((2 - c^n) Ud^{n-1/2} + 2 R^n / lam) / (2 + c^n)   (first iteration: R^0 / (2 lam));  U^{n+1} = U^n + Ud^{n+1/2}
+ * Clamped dofs keep U; dofs flagged PD_PRESC_* advance by value[dim*i+k] per iteration (a fixed displacement increment,
+ * PAPER.md:813); PD_BODY_FORCE values are force densities as in pd_step; the failure check of pd_step runs on every
+ * U^{n+1} when s_c > 0.  The handle must have been created with rho = 1 and dt = 1 (pseudo time; PD_ERR_ARG otherwise).
+ * lam >= lambda_max(K)/4 for stability (K: f = -K u).  Asynchronous: c^n is formed on the device; pd_get_u returns U^n. */
+PD_API int pd_adr_step(pd_sim *sim, int64_t niter, double lam);
+
 /* ---- the paper's own scheme, as an on-box comparison for the matrix-free path ----
  * pd_matrix_create assembles, on the device, the four global sparse matrices CE (Nb x d n), CTH (n x Nb), KTH (d n x n),
  * KE (d n x Nb) of Eqs. 2.7-2.10 in CSR (int64 row pointers, int32 columns, FP64 values), user

@@ -32,6 +32,7 @@ class ADROracle:
         self.f_prev = np.zeros((n, d))
         self.it = 0
         self.c_hist = []
+        self.near_total = 0        # bonds within 1e-9 relative of s_c at a failure check (reported, like PDOracle.near_total)
         fl = oracle.flags
         self.clamped = np.stack([(fl & (1 << k)) != 0 for k in range(d)], axis=1)
         self.presc = np.stack([(fl & (8 << k)) != 0 for k in range(d)], axis=1) & ~self.clamped
@@ -63,7 +64,7 @@ class ADROracle:
             self.c_hist.append(c)
             self.it += 1
             if o.s_c > 0.0 and np.isfinite(o.s_c):
-                o.break_bonds()
+                self.near_total += o.break_bonds()[1]
         o.damage()
         return o.u
 

@@ -72,6 +72,51 @@ __global__ void k_gather_scalar(int64_t npad, const int32_t *__restrict__ perm, 
   dst[uidx] = src[i];
 }
 
+
+// ---- adaptive dynamic relaxation (pd_adr_step, Underwood 1983 / Kilic & Madenci 2010) ----
+// The step kernels run with rho = 1, dt = 1 and v zeroed before the force pass, so v holds the total force density
+// R^n = f(U^n) + g b on return.  Then (pseudo time step 1, Lambda = lam I):
+//   1K_ii = -(R_i^n - R_i^{n-1}) / (lam Ud_i^{n-1/2}),   c^n = 2 sqrt((U . 1K U) / (U . U))   over the free dofs
+//   Ud^{n+1/2} = ((2 - c^n) Ud^{n-1/2} + 2 R^n / lam) / (2 + c^n)   (n = 0: R^0 / (2 lam));   U^{n+1} = U^n + Ud^{n+1/2}
+__global__ void k_adr_reduce(int64_t npad, int dim, const int32_t *__restrict__ perm, const uint8_t *__restrict__ flags, FieldView u,
+                             FieldView r, FieldView rprev, FieldView ud, double lam, double *scal) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  double num = 0.0, den = 0.0;
+  if (i < npad && perm[i] >= 0) {
+    const unsigned fl = flags[i];
+    for (int k = 0; k < dim; ++k) {
+      if (fl & ((1u << k) | (8u << k))) continue;   // clamped / prescribed dofs are not free
+      const double U = field_ref(u, npad, i, k), d = field_ref(ud, npad, i, k);
+      const double k1 = d != 0.0 ? -(field_ref(r, npad, i, k) - field_ref(rprev, npad, i, k)) / (lam * d) : 0.0;
+      num += U * k1 * U;
+      den += U * U;
+    }
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    num += __shfl_xor_sync(0xffffffffu, num, o);
+    den += __shfl_xor_sync(0xffffffffu, den, o);
+  }
+  if ((threadIdx.x & 31) == 0 && (num != 0.0 || den != 0.0)) { atomicAdd(&scal[0], num); atomicAdd(&scal[1], den); }
+}
+__global__ void k_adr_update(int64_t npad, int dim, const int32_t *__restrict__ perm, const uint8_t *__restrict__ flags, FieldView u,
+                             FieldView unext, FieldView r, FieldView rprev, FieldView ud, FieldView bval, double lam, int first,
+                             const double *__restrict__ scal) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= npad || perm[i] < 0) return;
+  double c = 0.0;
+  if (!first && scal[1] > 0.0 && scal[0] / scal[1] > 0.0) c = 2.0 * sqrt(scal[0] / scal[1]);
+  const unsigned fl = flags[i];
+  for (int k = 0; k < dim; ++k) {
+    const double R = field_ref(r, npad, i, k);
+    double d = first ? 0.5 * R / lam : ((2.0 - c) * field_ref(ud, npad, i, k) + 2.0 * R / lam) / (2.0 + c);
+    if (fl & (1u << k)) d = 0.0;                                   // clamped
+    else if (fl & (8u << k)) d = field_ref(bval, npad, i, k);      // prescribed displacement increment per iteration
+    field_ref(unext, npad, i, k) = field_ref(u, npad, i, k) + d;
+    field_ref(ud, npad, i, k) = d;
+    field_ref(rprev, npad, i, k) = R;
+  }
+}
+
 struct DevTmp {  // RAII temp allocation through the sim's allocator
   pd_sim *s;
   void *p;
@@ -353,6 +398,41 @@ int pd_step_timed(pd_sim *s, int64_t nsteps, double ms[2]) {
   }
   for (auto &e : ev) cudaEventDestroy(e);
   return rc;
+}
+
+int pd_adr_step(pd_sim *s, int64_t niter, double lam) {
+  if (!s || niter < 0 || !(lam > 0.0)) { pdi::set_error("bad argument"); return PD_ERR_ARG; }
+  if (s->rho != 1.0 || s->dt != 1.0) { pdi::set_error("pd_adr_step needs a handle created with rho = 1 and dt = 1 (pseudo time)"); return PD_ERR_ARG; }
+  const int dim = s->dim;
+  if (!s->adr_ud[0]) {
+    for (int k = 0; k < dim; ++k) {
+      s->adr_ud[k] = (double *)pdi::dev_alloc(s, sizeof(double) * s->npad);
+      s->adr_rprev[k] = (double *)pdi::dev_alloc(s, sizeof(double) * s->npad);
+      if (!s->adr_ud[k] || !s->adr_rprev[k]) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
+      cudaMemsetAsync(s->adr_ud[k], 0, sizeof(double) * s->npad, s->stream);
+      cudaMemsetAsync(s->adr_rprev[k], 0, sizeof(double) * s->npad, s->stream);
+    }
+    s->adr_scal = (double *)pdi::dev_alloc(s, 2 * sizeof(double));
+    if (!s->adr_scal) { pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
+  }
+  const FieldView ud = view_soa(s->adr_ud), rprev = view_soa(s->adr_rprev), r = view_soa(s->v), bval = view_soa(s->bval);
+  for (int64_t it = 0; it < niter; ++it) {
+    int rc = pdi::launch_dilatation(s, nullptr, s->break_pending);
+    if (rc) return rc;
+    for (int k = 0; k < dim; ++k) cudaMemsetAsync(s->v[k], 0, sizeof(double) * s->npad, s->stream);
+    if ((rc = pdi::launch_force_update(s))) return rc;   // v = R^n; the other u buffer is overwritten below
+    const int first = s->adr_it == 0;
+    const FieldView u = view_u(s, s->cur), unext = view_u(s, s->cur ^ 1);
+    if (!first) {
+      cudaMemsetAsync(s->adr_scal, 0, 2 * sizeof(double), s->stream);
+      k_adr_reduce<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, s->perm, s->flags, u, r, rprev, ud, lam, s->adr_scal);
+    }
+    k_adr_update<<<nblk(s->npad), TPB, 0, s->stream>>>(s->npad, dim, s->perm, s->flags, u, unext, r, rprev, ud, bval, lam, first,
+                                                       s->adr_scal);
+    s->cur ^= 1; s->step += 1; s->adr_it += 1; s->break_pending = s->fracture; s->launches += 2;
+  }
+  PD_CUDA(cudaGetLastError());
+  return PD_OK;
 }
 
 int pd_get_u(pd_sim *s, double *dst) { return s ? get_field(s, dst, false) : PD_ERR_ARG; }

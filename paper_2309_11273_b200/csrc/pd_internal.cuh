@@ -181,6 +181,9 @@ struct pd_sim {
   cudaGraphExec_t graph[2] = {nullptr, nullptr};
   cudaStream_t cap_stream = nullptr;
   unsigned long long *stats_dev = nullptr;  // [0]=broken directed, [1]=max phi bits, [2]=#phi>=.5
+  // adaptive dynamic relaxation (pd_adr_step): Ud^{n-1/2}, R^{n-1} (SoA, internal component order), {num, den} of c^n
+  double *adr_ud[PD_MAX_DIM] = {}, *adr_rprev[PD_MAX_DIM] = {}, *adr_scal = nullptr;
+  int64_t adr_it = 0;
 };
 
 namespace pdi {

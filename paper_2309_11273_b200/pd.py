@@ -18,7 +18,7 @@ _LIBPATH = os.environ.get("PD_LIBPATH") or os.path.join(_HERE, "libpd.so")   # P
 PD_OK, PD_ERR_ARG, PD_ERR_ISOLATED, PD_ERR_ALLOC, PD_ERR_CUDA, PD_ERR_LIMIT = 0, -1, -2, -3, -4, -5
 EXPORTS = ["pd_create", "pd_step", "pd_get_u", "pd_get_v", "pd_get_damage", "pd_destroy", "pd_get_stats",
            "pd_get_bond_mask", "pd_get_node_fields", "pd_get_layout", "pd_step_timed", "pd_last_error", "pd_version",
-           "pd_matrix_create", "pd_matrix_step", "pd_matrix_get", "pd_matrix_destroy"]
+           "pd_matrix_create", "pd_matrix_step", "pd_matrix_get", "pd_matrix_destroy", "pd_adr_step"]
 
 
 class PdMaterial(C.Structure):
@@ -74,6 +74,7 @@ def load():
         lib.pd_matrix_create.argtypes = [C.POINTER(C.c_void_p), C.c_int64, C.c_void_p, C.c_void_p, C.POINTER(PdMaterial),
                                          C.POINTER(PdBoundary), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.pd_matrix_step.argtypes = [C.c_void_p, C.c_int64]
+        lib.pd_adr_step.argtypes = [C.c_void_p, C.c_int64, C.c_double]
         lib.pd_matrix_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.pd_matrix_destroy.argtypes = [C.c_void_p]
         _lib = lib
@@ -203,6 +204,10 @@ class Sim:
                 raise ValueError(f"out must be a contiguous float64 array of {n} elements on the host or on {self.device}")
         self._ck(fn(self.h, _ptr(out)))
         return out
+
+    def adr_step(self, niter, lam):
+        """niter iterations of adaptive dynamic relaxation (pd_adr_step); the handle must have rho = 1, dt = 1"""
+        self._ck(self.lib.pd_adr_step(self.h, int(niter), float(lam)))
 
     def get_u(self, out=None):
         return self._get(self.lib.pd_get_u, (self.n, self.dim), out)

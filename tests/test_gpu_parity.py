@@ -349,3 +349,79 @@ def test_matrix_scheme_matches_oracle():
         assert _rel(u, o.u) <= TOL and _rel(v, o.v) <= TOL, wl.name
         assert _rel(u, sim.get_u()) <= TOL
         ms.destroy(); sim.destroy()
+
+
+@pytest.mark.parametrize("env", [{}, {"PD_LAT_UNIFORM": "0"}, {"PD_FORCE_GENERIC": "1"}])
+def test_adr_quasi_static_driver(env, monkeypatch):
+    """adaptive dynamic relaxation (pd_adr_step) against the oracle's ADR (oracle/pd_adr.py,
+    itself pinned to the direct solve).  The damping estimate c^n divides force differences by velocities that pass
+    through zero, so two correct implementations drift apart in their ITERATES after some tens of iterations (measured:
+    1e-14 after 8 iterations, 1e-3 after 50 under continuous displacement loading) while converging to the same
+    equilibrium; the test therefore checks (a) iterate-by-iterate equality while it holds, on a smooth load for hundreds
+    of iterations; (b) a failure check inside the first iterations: identical broken sets; (c) the converged states."""
+    from paper_2309_11273_b200 import pd
+    from oracle.pd_oracle import PDOracle
+    from oracle.pd_adr import ADROracle
+    for k in _ENV_KEYS:
+        monkeypatch.delenv(k, raising=False)
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    # (a) bar 14 x 6 x 5 cells, one end clamped, body force on the other end layer
+    g = np.stack(np.meshgrid(np.arange(14), np.arange(6), np.arange(5), indexing="ij"), -1).reshape(-1, 3)
+    x = (g + 0.5) * 1e-3
+    fl = np.zeros(len(x), np.uint8); fl[g[:, 0] < 2] = 7; fl[g[:, 0] == 13] |= 64
+    val = np.zeros_like(x); val[g[:, 0] == 13] = [3e9, 5e8, 0.0]
+    kw = dict(dim=3, mode=0, E=72e9, nu=0.22, rho=1.0, dt=1.0)
+    vol = np.full(len(x), 1e-9)
+    lam = 0.3 * 72e9 / 1e-6          # >= lambda_max(K)/4 for this lattice (the run stays bounded and converges)
+    o = PDOracle(x, vol, 3.015e-3, **kw, flags=fl, value=val)
+    adr = ADROracle(o, lam)
+    sim = pd.Sim(x, vol, 3.015e-3, **kw, flags=fl, value=val)
+    for chunk in (1, 2, 40, 300):
+        adr.iterate(chunk); sim.adr_step(chunk, lam)
+        assert _rel(sim.get_u(), o.u) <= 1e-9, chunk
+    assert np.abs(o.u).max() > 1e-7 and max(adr.c_hist) > 0
+    sim.destroy()
+    # plate 40 x 24 with a pre-notch; top and bottom rows driven apart by a fixed increment per iteration
+    nx, ny, dx = 40, 24, 1e-3
+    gx, gy = np.meshgrid(np.arange(nx), np.arange(ny), indexing="xy")
+    gx, gy = gx.reshape(-1), gy.reshape(-1)
+    x = np.stack([(gx + 0.5) * dx, (gy + 0.5) * dx], 1)
+    fl = np.zeros(nx * ny, np.uint8); val = np.zeros((nx * ny, 2))
+    fl[gy >= ny - 3] = 8 | 16; val[gy >= ny - 3, 1] = +2e-9
+    fl[gy < 3] = 8 | 16; val[gy < 3, 1] = -2e-9
+    from paper_2309_11273_b200.workloads import _precut_horizontal
+    precut = _precut_horizontal(nx, ny, ny // 2, 2 * (nx // 3))
+    vol = np.full(nx * ny, dx * dx * 1e-3)
+    lam = 0.3 * 72e9 / dx ** 2
+    # (b) s_c so small that the bonds next to the driven rows break in iterations 4-8 (stretch 2e-6 per iteration)
+    kw = dict(dim=2, mode=1, E=72e9, nu=0.22, rho=1.0, dt=1.0, s_c=7e-6)
+    o = PDOracle(x, vol, 3.015 * dx, **kw, flags=fl, value=val, precut=precut)
+    adr = ADROracle(o, lam)
+    sim = pd.Sim(x, vol, 3.015 * dx, **kw, flags=fl, value=val, precut=precut)
+    for chunk in (3, 2, 3):
+        adr.iterate(chunk); sim.adr_step(chunk, lam)
+        bs, _, _ = _broken_set(sim)
+        assert adr.near_total == 0, "near-threshold events must be reported"
+        assert bs == o.broken_set(), (len(bs), len(o.broken_set()))
+        assert _rel(sim.get_u(), o.u) <= 1e-10
+        assert np.allclose(sim.get_damage(), o.damage(), rtol=0, atol=1e-12)
+    assert len(o.broken_set()) > 2 * len(precut), "the case must actually break bonds"
+    sim.destroy()
+    # (c) no failure: 100 increments, then hold and relax: both reach the same equilibrium
+    kw["s_c"] = 0.0
+    o = PDOracle(x, vol, 3.015 * dx, **kw, flags=fl, value=val, precut=precut)
+    adr = ADROracle(o, lam)
+    sim = pd.Sim(x, vol, 3.015 * dx, **kw, flags=fl, value=val, precut=precut)
+    adr.iterate(100); sim.adr_step(100, lam)
+    sim.destroy()
+    u_hold = o.u.copy()
+    o2 = PDOracle(x, vol, 3.015 * dx, **kw, flags=fl, value=np.zeros_like(val), precut=precut, u0=u_hold)
+    # (prescribed dofs keep the displacement reached; increments are zero from here on)
+    adr2 = ADROracle(o2, lam)
+    sim2 = pd.Sim(x, vol, 3.015 * dx, **kw, flags=fl, value=np.zeros_like(val), precut=precut, u0=u_hold)
+    adr2.iterate(2500); sim2.adr_step(2500, lam)
+    assert _rel(sim2.get_u(), o2.u) <= 1e-6
+    r = np.abs(adr2.total_force()[(fl & 24) == 0]).max()       # residual on the free dofs at the oracle's end state
+    assert r <= 1e-6 * np.abs(adr2.o.force_density()).max()
+    sim2.destroy()
