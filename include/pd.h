@@ -178,6 +178,15 @@ PD_API int pd_get_layout(pd_sim *sim, int64_t counts[8]);
  * ms[0] = dilatation(+break) kernel, ms[1] = force+update kernel.  Synchronises. */
 PD_API int pd_step_timed(pd_sim *sim, int64_t nsteps, double ms[2]);
 
+/* ---- halo pack / unpack of the multi-GPU slab decomposition (paper_2309_11273_b200/slabs.py) ----
+ * pd_gather_u copies the rows idx[0..count) (user node indices) of the current displacement u^n into dst (count*dim doubles,
+ * AoS); pd_scatter_u overwrites those rows of u^n with src.  idx, dst, src are DEVICE pointers (the buffers that the
+ * point-to-point exchange between slab neighbours sends and receives); both calls are asynchronous on the handle's
+ * stream and do not touch v or the bond status.  Between two pd_step calls a rank gathers the owned nodes its
+ * neighbours hold as halo, exchanges, and scatters the halo nodes it received: that is the whole exchange step. */
+PD_API int pd_gather_u(pd_sim *sim, const int32_t *idx, int64_t count, double *dst);
+PD_API int pd_scatter_u(pd_sim *sim, const int32_t *idx, int64_t count, const double *src);
+
 /* ---- quasi-static driver: adaptive dynamic relaxation ----
  * The paper solves its Ex. 4 "by using an adaptive dynamic relaxation algorithm presented in [Underwood 1983; Kilic &
  * Madenci 2010]" and does not restate it; this is that algorithm with a uniform fictitious density

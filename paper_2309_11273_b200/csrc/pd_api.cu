@@ -51,6 +51,18 @@ __global__ void k_gather_field(int64_t npad, int dim, Ax ax, const int32_t *__re
   for (int k = 0; k < dim; ++k) dst[(int64_t)dim * uidx + ax.a[k]] = field_ref(f, npad, i, k);
 }
 
+// halo pack / unpack of the slab decomposition: rows idx[q] (user indices) of u <-> a dense (count x dim) AoS buffer
+__global__ void k_pack_u(int64_t count, int dim, Ax ax, int64_t npad, const int32_t *__restrict__ idx, const int32_t *__restrict__ iperm,
+                         FieldView u, double *buf, bool unpack) {
+  int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= count) return;
+  const int64_t i = iperm[idx[q]];
+  for (int k = 0; k < dim; ++k) {
+    if (unpack) field_ref(u, npad, i, k) = buf[q * dim + ax.a[k]];
+    else buf[q * dim + ax.a[k]] = field_ref(u, npad, i, k);
+  }
+}
+
 FieldView view_u(pd_sim *s, int buf) {
   FieldView f{};
   if (s->lat.on && s->lat.uniform) { f.uxy = s->lat.uxy[buf]; f.uz = s->lat.uz[buf]; }
@@ -398,6 +410,24 @@ int pd_step_timed(pd_sim *s, int64_t nsteps, double ms[2]) {
   }
   for (auto &e : ev) cudaEventDestroy(e);
   return rc;
+}
+
+int pd_gather_u(pd_sim *s, const int32_t *idx, int64_t count, double *dst) {
+  if (!s || count < 0 || (count > 0 && (!idx || !dst))) { pdi::set_error("bad argument"); return PD_ERR_ARG; }
+  if (count == 0) return PD_OK;
+  k_pack_u<<<nblk(count), TPB, 0, s->stream>>>(count, s->dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->npad, idx, s->iperm,
+                                               view_u(s, s->cur), dst, false);
+  PD_CUDA(cudaGetLastError());
+  return PD_OK;
+}
+
+int pd_scatter_u(pd_sim *s, const int32_t *idx, int64_t count, const double *src) {
+  if (!s || count < 0 || (count > 0 && (!idx || !src))) { pdi::set_error("bad argument"); return PD_ERR_ARG; }
+  if (count == 0) return PD_OK;
+  k_pack_u<<<nblk(count), TPB, 0, s->stream>>>(count, s->dim, Ax{{s->ax[0], s->ax[1], s->ax[2]}}, s->npad, idx, s->iperm,
+                                               view_u(s, s->cur), const_cast<double *>(src), true);
+  PD_CUDA(cudaGetLastError());
+  return PD_OK;
 }
 
 int pd_adr_step(pd_sim *s, int64_t niter, double lam) {

@@ -18,7 +18,8 @@ _LIBPATH = os.environ.get("PD_LIBPATH") or os.path.join(_HERE, "libpd.so")   # P
 PD_OK, PD_ERR_ARG, PD_ERR_ISOLATED, PD_ERR_ALLOC, PD_ERR_CUDA, PD_ERR_LIMIT = 0, -1, -2, -3, -4, -5
 EXPORTS = ["pd_create", "pd_step", "pd_get_u", "pd_get_v", "pd_get_damage", "pd_destroy", "pd_get_stats",
            "pd_get_bond_mask", "pd_get_node_fields", "pd_get_layout", "pd_step_timed", "pd_last_error", "pd_version",
-           "pd_matrix_create", "pd_matrix_step", "pd_matrix_get", "pd_matrix_destroy", "pd_adr_step"]
+           "pd_matrix_create", "pd_matrix_step", "pd_matrix_get", "pd_matrix_destroy", "pd_adr_step",
+           "pd_gather_u", "pd_scatter_u"]
 
 
 class PdMaterial(C.Structure):
@@ -75,6 +76,8 @@ def load():
                                          C.POINTER(PdBoundary), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.pd_matrix_step.argtypes = [C.c_void_p, C.c_int64]
         lib.pd_adr_step.argtypes = [C.c_void_p, C.c_int64, C.c_double]
+        lib.pd_gather_u.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
+        lib.pd_scatter_u.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
         lib.pd_matrix_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.pd_matrix_destroy.argtypes = [C.c_void_p]
         _lib = lib
@@ -204,6 +207,31 @@ class Sim:
                 raise ValueError(f"out must be a contiguous float64 array of {n} elements on the host or on {self.device}")
         self._ck(fn(self.h, _ptr(out)))
         return out
+
+    def _dev_idx(self, idx):
+        """device copy (int32) of an index list, cached per list object"""
+        import torch
+        cache = self.__dict__.setdefault("_idx_cache", {})
+        key = id(idx)
+        if key not in cache:
+            cache[key] = (idx, torch.as_tensor(np.ascontiguousarray(idx, dtype=np.int32), device=self.device))
+        return cache[key][1]
+
+    def gather_u(self, idx):
+        """rows idx (user indices) of u^n as a (len(idx), dim) float64 tensor on the handle's device (pd_gather_u)"""
+        import torch
+        di = self._dev_idx(idx)
+        out = torch.empty((di.numel(), self.dim), dtype=torch.float64, device=self.device)
+        self._ck(self.lib.pd_gather_u(self.h, di.data_ptr(), di.numel(), out.data_ptr()))
+        return out
+
+    def scatter_u(self, idx, values):
+        """overwrite rows idx of u^n with values ((len(idx), dim), tensor on the device or array) (pd_scatter_u)"""
+        import torch
+        di = self._dev_idx(idx)
+        v = torch.as_tensor(values, dtype=torch.float64, device=self.device).contiguous()
+        assert v.numel() == di.numel() * self.dim
+        self._ck(self.lib.pd_scatter_u(self.h, di.data_ptr(), di.numel(), v.data_ptr()))
 
     def adr_step(self, niter, lam):
         """niter iterations of adaptive dynamic relaxation (pd_adr_step); the handle must have rho = 1, dt = 1"""
