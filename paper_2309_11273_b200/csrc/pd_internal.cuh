@@ -133,8 +133,12 @@ struct PdLattice {
   int32_t *off2bit = nullptr;      // [(2S2+1)(2S1+1)(2S0+1)] offset -> bit index or -1
   double r2lb[128];                // per stencil bit: min over all bonds of ||xi||^2 exactly as the step kernels
                                    // compute it (break-test filter: dot < s_c * r2lb  =>  the bond cannot break)
-  void *cache[4] = {nullptr, nullptr, nullptr, nullptr};   // host: prepared launch arguments of the step kernels
-                                   // ([0], [1]: pd_lattice_uniform.cu; [2], [3]: pd_lattice_step.cu)
+  void *cache[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // host: prepared launch arguments of the step
+                                   // kernels ([0], [1]: pd_lattice_uniform.cu; [2], [3]: pd_lattice_step.cu; [4], [5]: pd_lattice_ball.cu)
+  // pd_lattice_ball.cu: octant words of mask / nofail [8][npad] and the exact-pass tables (device)
+  uint32_t *mask8 = nullptr, *nf8 = nullptr;
+  void *ball_btab = nullptr, *ball_boff = nullptr, *ball_q8 = nullptr;
+  uint8_t *ball_tfull = nullptr;   // per warp tile: every family complete, intact and allowed to break
   int32_t *thr_dir = nullptr;      // device: per (column, step) filter thresholds of the dilatation kernel (pd_lattice_step.cu)
   int S[3] = {0, 0, 0};
 };
@@ -210,6 +214,10 @@ void lat_free_cache(pd_sim *s);
 int ulat_launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
 int ulat_launch_force_update(pd_sim *s);
 void ulat_free_cache(pd_sim *s);
+// pd_lattice_ball.cu: return 1 if launched, 0 if the lattice's stencil is not the compiled-in ball
+int ball_launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
+int ball_launch_force_update(pd_sim *s);
+void ball_free_cache(pd_sim *s);
 // pd_step.cu
 int launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
 int launch_force_update(pd_sim *s);

@@ -32,7 +32,6 @@
 //     compile-time offset from one shared-memory pointer.
 //   DIRECT (stencils wider than the staged halo, or no tensor maps): records are read from the dense
 //     arrays by arithmetic addressing through L1, as in pd_lattice_step.cu.
-#include <cuda.h>   // CUtensorMap (types only; the encoder is fetched through cudaGetDriverEntryPoint)
 
 #include <algorithm>
 #include <cmath>
@@ -42,8 +41,11 @@
 #include <vector>
 
 #include "pd_internal.cuh"
+#include "pd_stage.cuh"
 
 namespace {
+
+using namespace pdstage;
 
 constexpr unsigned FULL = 0xffffffffu;
 constexpr int UH = 3;              // STAGED kernels: halo of a staged plane = largest stencil radius in x and y they take
@@ -89,26 +91,6 @@ struct UArgs {
   double A, c1, G, vol_uniform, rrho, dt, gramp;   // gramp = g(t_n) = min(1, n dt / ramp_time)
   alignas(64) CUtensorMap tm_xy, tm_z, tm_g;       // STAGED: 3-D tiled maps of uxy (as doubles), uz, aux (as doubles)
 };
-
-// ---- mbarrier / TMA (sm_90+ PTX) ----
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\tWAIT_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
-      ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-// one plane box (c0 = innermost coordinate) -> shared memory; completes on the mbarrier
-__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *tm, int c0, int c1, int c2, uint64_t *bar) {
-  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-               ::"r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
-}
 
 // predicated read-only loads: no branch, so the bonds of a step stay in one basic block
 __device__ __forceinline__ void ldg2_if(double2 &v, const double2 *ptr, uint32_t pred) {
@@ -537,27 +519,6 @@ struct UPrepared {
   CUtensorMap tm_xy[2], tm_z[2], tm_g;   // per displacement buffer
 };
 
-// 3-D tiled tensor map over a dense cell array viewed as doubles (epc doubles per cell), box = USX cells x sy rows x 1 level
-typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
-                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-bool make_plane_map(CUtensorMap *tm, void *base, int epc, int DX, int DY, int DZ, int sy) {
-  static EncodeTiledFn encode = nullptr;
-  if (!encode) {
-    void *fn = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
-        qres != cudaDriverEntryPointSuccess) { cudaGetLastError(); return false; }
-    encode = (EncodeTiledFn)fn;
-  }
-  const cuuint64_t dims[3] = {(cuuint64_t)DX * epc, (cuuint64_t)DY, (cuuint64_t)DZ};
-  const cuuint64_t strides[2] = {(cuuint64_t)DX * epc * 8, (cuuint64_t)DX * DY * epc * 8};   // bytes, dims 1 and 2
-  const cuuint32_t box[3] = {(cuuint32_t)(USX * epc), (cuuint32_t)sy, 1u};
-  const cuuint32_t estr[3] = {1u, 1u, 1u};
-  return encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
-
 // device tables: per stencil bit {xi_1, thr = s_c ||xi||^2} (dilatation) or {xi_1, 1 / ||xi||^2} (force), ||xi||^2 in the
 // kernels' own operation order; per column the UCol record (xi_0, xi_2 are constant along a column)
 bool ulat_tables(pd_sim *s, bool force, UArgs &a) {
@@ -662,10 +623,10 @@ UPrepared *ulat_prepare(pd_sim *s, bool force, bool allow_staged = true) {
   if (pp->staged) {
     bool ok = true;
     for (int q = 0; q < 2 && ok; ++q) {
-      ok = make_plane_map(&pp->tm_xy[q], l.uxy[q], 2, l.DX, l.DY, l.DZ, a.sy);
-      if (ok && s->dim == 3) ok = make_plane_map(&pp->tm_z[q], l.uz[q], 1, l.DX, l.DY, l.DZ, a.sy);
+      ok = make_plane_map(&pp->tm_xy[q], l.uxy[q], 2, l.DX, l.DY, l.DZ, USX, a.sy);
+      if (ok && s->dim == 3) ok = make_plane_map(&pp->tm_z[q], l.uz[q], 1, l.DX, l.DY, l.DZ, USX, a.sy);
     }
-    if (ok) ok = make_plane_map(&pp->tm_g, l.aux, 2, l.DX, l.DY, l.DZ, a.sy);
+    if (ok) ok = make_plane_map(&pp->tm_g, l.aux, 2, l.DX, l.DY, l.DZ, USX, a.sy);
     if (!ok || pp->smem > 232448 - 1024) {   // no tensor maps on this driver / planes do not fit: the direct variant
       delete pp;
       return ulat_prepare(s, force, false);
@@ -710,6 +671,7 @@ void ulat_dispatch(const UPrepared *pp, cudaStream_t st) {
 namespace pdi {
 
 void ulat_free_cache(pd_sim *s) {
+  ball_free_cache(s);
   for (int q = 0; q < 2; ++q) {
     delete (UPrepared *)s->lat.cache[q];
     s->lat.cache[q] = nullptr;
@@ -717,6 +679,7 @@ void ulat_free_cache(pd_sim *s) {
 }
 
 int ulat_launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
+  if (ball_launch_dilatation(s, theta_out, do_break)) return PD_OK;   // the compiled-in 122-offset stencil
   UPrepared *pp = ulat_prepare(s, false);
   if (!pp) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
   const PdLattice &l = s->lat;
@@ -731,6 +694,7 @@ int ulat_launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
 }
 
 int ulat_launch_force_update(pd_sim *s) {
+  if (ball_launch_force_update(s)) return PD_OK;
   UPrepared *pp = ulat_prepare(s, true);
   if (!pp) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
   const PdLattice &l = s->lat;

@@ -178,14 +178,15 @@ def impact2d(nx=400, ny=400, steps=3000, vbar=16.5) -> Workload:
 
 
 # ---- config 4 ------------------------------------------------------------------------------
-def block3d(nx=200, ny=40, nz=40, steps=1000, seed=4321, amp=1e-5) -> Workload:
-    """Config 4: 3D cantilever block, jittered lattice, bending + torsion start (C-18)."""
+def block3d(nx=200, ny=40, nz=40, steps=1000, seed=4321, amp=1e-5, jitter=1e-3) -> Workload:
+    """Config 4: 3D cantilever block, jittered lattice (jitter = 0: plain lattice), bending + torsion start (C-18)."""
     dx = 1e-3
     iz, iy, ix = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
     ix, iy, iz = ix.reshape(-1), iy.reshape(-1), iz.reshape(-1)   # id = (iz*ny + iy)*nx + ix
     n = nx * ny * nz
     coords = np.stack([(ix + 0.5) * dx, (iy + 0.5) * dx, (iz + 0.5) * dx], axis=1)
-    coords = coords + np.random.default_rng(seed).uniform(-1e-3 * dx, 1e-3 * dx, size=(n, 3))
+    if jitter != 0.0:
+        coords = coords + np.random.default_rng(seed).uniform(-jitter * dx, jitter * dx, size=(n, 3))
     L, yc, zc, Rh = nx * dx, 0.5 * ny * dx, 0.5 * nz * dx, 0.5 * ny * dx
     x, y, z = coords[:, 0], coords[:, 1], coords[:, 2]
     u0 = np.zeros((n, 3))
@@ -198,7 +199,7 @@ def block3d(nx=200, ny=40, nz=40, steps=1000, seed=4321, amp=1e-5) -> Workload:
     return Workload("block3d", 3, MODE_3D, coords, np.full(n, dx ** 3), M_RATIO * dx, **GLASS, s_c=0.0,
                     dt=sc["dt"], ramp_time=0.0, flags=flags, value=np.zeros((n, 3)),
                     precut=np.zeros((0, 2), np.int32), u0=u0, v0=np.zeros((n, 3)), steps=steps, dx=dx,
-                    meta=dict(nx=nx, ny=ny, nz=nz))
+                    meta=dict(nx=nx, ny=ny, nz=nz, jitter=jitter))
 
 
 # ---- config 5 / 5' -------------------------------------------------------------------------

@@ -20,16 +20,20 @@ LAYOUTS = {
     "default": ({}, None),
     # uniform lattice, records through L1 instead of TMA-staged planes; rows per lane swapped (2 in 3-D, 4 in 2-D);
     # plain launches instead of CUDA graphs
-    "uniform_direct": ({"PD_ULAT_STAGED": "0", "PD_ULAT_DIL_ROWS": "-1", "PD_ULAT_FRC_ROWS": "-1", "PD_GRAPH": "0"}, None),
+    # (PD_BALL=0: the table-driven kernels also where the stencil is the compiled-in 122-offset ball of pd_lattice_ball.cu)
+    "uniform_direct": ({"PD_ULAT_STAGED": "0", "PD_ULAT_DIL_ROWS": "-1", "PD_ULAT_FRC_ROWS": "-1", "PD_GRAPH": "0",
+                        "PD_BALL": "0"}, None),
     # staged planes with 3 buffers in flight, rows per lane swapped, 2 row groups per CTA
     "uniform_nb3": ({"PD_ULAT_NB": "3", "PD_ULAT_DIL_ROWS": "-1", "PD_ULAT_FRC_ROWS": "-1", "PD_ULAT_DIL_CY": "2",
-                     "PD_ULAT_FRC_CY": "2"}, None),
+                     "PD_ULAT_FRC_CY": "2", "PD_BALL": "0"}, None),
+    # table-driven staged kernels with their default shape
+    "uniform_table": ({"PD_BALL": "0"}, None),
     "lattice_general": ({"PD_LAT_UNIFORM": "0"}, 1),
     "lattice_general_2rows": ({"PD_LAT_UNIFORM": "0", "PD_DIR_DIL_ROWS": "2", "PD_DIR_FRC_ROWS": "2"}, 1),
     "sliced_ell": ({"PD_FORCE_GENERIC": "1"}, 0),
 }
 _ENV_KEYS = ("PD_LAT_UNIFORM", "PD_FORCE_GENERIC", "PD_DIR_DIL_ROWS", "PD_DIR_FRC_ROWS", "PD_ULAT_DIL_ROWS",
-             "PD_ULAT_FRC_ROWS", "PD_ULAT_STAGED", "PD_ULAT_NB", "PD_ULAT_DIL_CY", "PD_ULAT_FRC_CY", "PD_GRAPH")
+             "PD_ULAT_FRC_ROWS", "PD_ULAT_STAGED", "PD_ULAT_NB", "PD_ULAT_DIL_CY", "PD_ULAT_FRC_CY", "PD_GRAPH", "PD_BALL")
 
 
 @pytest.fixture(params=list(LAYOUTS))
@@ -46,7 +50,7 @@ def _expect_layout(code, wl):
     """the layout pd_create must pick by itself: jittered lattices cannot take the uniform path"""
     if code is not None:
         return code
-    return 1 if wl.name == "block3d" else 2
+    return 1 if wl.name == "block3d" and wl.meta.get("jitter", 1.0) != 0.0 else 2
 
 
 def _oracle(wl):
@@ -79,10 +83,14 @@ def _small_cases():
         "config3_small": (W.impact2d(nx=72, ny=72), 500),
         "config4_small": (W.block3d(nx=37, ny=13, nz=11), 120),          # ragged: 5291 nodes, not /32
         "config5_small": (W.cylinder3d(r_cells=9, l_cells=34, omega=400.0), 300),   # omega raised so the short run breaks bonds
+        # long enough along the lane axis for row groups with every family complete (the FAST bodies of the
+        # compiled-in stencil, their break filter and exact pass), ragged last chunk
+        "config5_long": (W.cylinder3d(r_cells=9, l_cells=100, omega=400.0), 300),
+        "block3d_uniform": (W.block3d(nx=70, ny=13, nz=11, jitter=0.0), 120),       # unjittered: uniform lattice, no fracture
     }
 
 
-@pytest.mark.parametrize("name", ["config1_full", "config4_small"])
+@pytest.mark.parametrize("name", ["config1_full", "config4_small", "block3d_uniform"])
 def test_no_fracture_trajectory(name, layout):
     wl, nsteps = _small_cases()[name]
     sim, o = _sim(wl), _oracle(wl)
@@ -103,7 +111,7 @@ def test_no_fracture_trajectory(name, layout):
     sim.destroy()
 
 
-@pytest.mark.parametrize("name", ["config2_small", "config3_small", "config5_small"])
+@pytest.mark.parametrize("name", ["config2_small", "config3_small", "config5_small", "config5_long"])
 def test_fracture_broken_sets(name, layout):
     wl, nsteps = _small_cases()[name]
     sim, o = _sim(wl), _oracle(wl)
