@@ -171,6 +171,10 @@ struct BState {
 __device__ __forceinline__ void prefetch_l1(const void *ptr) { asm volatile("prefetch.global.L1 [%0];" ::"l"(ptr)); }
 __device__ __forceinline__ void keep(double &v) { asm volatile("" : "+d"(v)); }
 __device__ __forceinline__ void keep(int &v) { asm volatile("" : "+r"(v)); }
+// x or -x by flipping the sign bit on the integer pipe (neg = 0 or 0x80000000)
+__device__ __forceinline__ double signed_const(double x, int neg) {
+  return __hiloint2double(__double2hiint(x) ^ neg, __double2loint(x));
+}
 struct BSign {
   double xs0[4], xs1[4], xs2[4];   // sx a h_0, sy b h_1, sz c h_2
   int ry[4], cx[4];                // byte offsets inside the staged xy plane: sy b BSX 16, sx a 16
@@ -398,7 +402,7 @@ __global__ void __launch_bounds__(CY * 32, MINB) k_ball(const __grid_constant__ 
     if (active) {
       if (mz) swap_levels<RZ>(p, FORCE);   // z -> -z: the lane's levels change places
 #pragma unroll
-      for (int c = 1; c < 4; ++c) { sg.xs2[c] = mz ? -a.xi[2][c] : a.xi[2][c]; keep(sg.xs2[c]); }
+      for (int c = 1; c < 4; ++c) { sg.xs2[c] = signed_const(a.xi[2][c], mz << 31); keep(sg.xs2[c]); }
     }
     sfor<0, NP / 2>([&](auto Jc) {
       constexpr int J = CV(Jc);
@@ -412,7 +416,7 @@ __global__ void __launch_bounds__(CY * 32, MINB) k_ball(const __grid_constant__ 
         for (int my = 0; my < 2; ++my) {
 #pragma unroll
           for (int c = 1; c < 4; ++c) {
-            sg.xs1[c] = my ? -a.xi[1][c] : a.xi[1][c]; sg.ry[c] = (my ? -c : c) * (BSX * 16);
+            sg.xs1[c] = signed_const(a.xi[1][c], my << 31); sg.ry[c] = (my ? -c : c) * (BSX * 16);
             keep(sg.xs1[c]); keep(sg.ry[c]);
           }
           sg.ry[0] = 0;
@@ -420,7 +424,7 @@ __global__ void __launch_bounds__(CY * 32, MINB) k_ball(const __grid_constant__ 
           for (int mx = 0; mx < 2; ++mx) {
 #pragma unroll
             for (int c = 1; c < 4; ++c) {
-              sg.xs0[c] = mx ? -a.xi[0][c] : a.xi[0][c]; sg.cx[c] = (mx ? -c : c) * 16;
+              sg.xs0[c] = signed_const(a.xi[0][c], mx << 31); sg.cx[c] = (mx ? -c : c) * 16;
               keep(sg.xs0[c]); keep(sg.cx[c]);
             }
             sg.cx[0] = 0;
