@@ -304,12 +304,13 @@ __global__ void __launch_bounds__(CY * 32, MINB) k_ball(const __grid_constant__ 
       if (z0 + l < a.PZ) active |= a.rgocc[((int64_t)(z0 + l) * a.nyq + (y0 >> 2)) * a.nxc + xc] != 0;
   }
   if (!__syncthreads_or(active)) return;   // barriers visible; nothing to do for the whole CTA?
-  // the planes are consumed in the order 0 .. NP/2 - 1, NP - 1 .. NP/2; position k of that order holds the box
+  // the planes are consumed in the order NP/2 - 1 .. 0, NP/2 .. NP - 1 (the planes with most bonds first in each half,
+  // so their walk hides the next loads); position k of that order holds the box
   // [xc 32 + HX - S, +BSX) x [yt + HY - S, +sy) of level z0 + HZ - S + plane(k)
   auto issue = [&](int k) {
     const int b = k % NB;
     unsigned char *dst = smraw + SM::o_buf + b * SM::plane;
-    const int plane = k >= NP / 2 ? NP - 1 - (k - NP / 2) : k;
+    const int plane = k < NP / 2 ? NP / 2 - 1 - k : k;
     const int cx = xc * 32 + a.HX - S, cyy = blockIdx.y * CY + a.HY - S, czz = z0 + a.HZ - S + plane;
     mbar_expect_tx(&full[b], SM::tx);
     tma_load_3d(dst, &a.tm_xy, 2 * cx, cyy, czz, &full[b]);
@@ -405,8 +406,8 @@ __global__ void __launch_bounds__(CY * 32, MINB) k_ball(const __grid_constant__ 
       for (int c = 1; c < 4; ++c) { sg.xs2[c] = signed_const(a.xi[2][c], mz << 31); keep(sg.xs2[c]); }
     }
     sfor<0, NP / 2>([&](auto Jc) {
-      constexpr int J = CV(Jc);
-      const int k = mz * (NP / 2) + J, b = k % NB;
+      constexpr int J = NP / 2 - 1 - CV(Jc);   // plane J of the first half, or its mirror image NP - 1 - J
+      const int k = mz * (NP / 2) + CV(Jc), b = k % NB;
       if (k > 0) leave(k);
       mbar_wait(&full[b], (k / NB) & 1);
       if (active) {
