@@ -137,7 +137,8 @@ struct PdLattice {
                                    // kernels ([0], [1]: pd_lattice_uniform.cu; [2], [3]: pd_lattice_step.cu; [4], [5]: pd_lattice_ball.cu)
   // pd_lattice_ball.cu: octant words of mask / nofail [8][npad] and the exact-pass tables (device)
   uint32_t *mask8 = nullptr, *nf8 = nullptr;
-  void *ball_btab = nullptr, *ball_boff = nullptr, *ball_q8 = nullptr;
+  void *ball_q8 = nullptr, *ball_wl = nullptr;   // table of the octant copies; worklist of the break test
+  int *ball_wl_count = nullptr;
   uint8_t *ball_tfull = nullptr;   // per warp tile: every family complete, intact and allowed to break
   int32_t *thr_dir = nullptr;      // device: per (column, step) filter thresholds of the dilatation kernel (pd_lattice_step.cu)
   int S[3] = {0, 0, 0};

@@ -123,7 +123,6 @@ __device__ __forceinline__ void sfor(F &&f) {
 }
 #define CV(x) (std::remove_reference_t<decltype(x)>::value)
 
-struct BTab { double xi0, xi1, xi2, thr; };   // exact pass: per mask bit
 
 struct BArgs {
   int DX, DY, PY, PZ, HX, HY, HZ;
@@ -142,17 +141,29 @@ struct BArgs {
   uint8_t *tfull;                    // [PZ / RZ][PY][nxc] 1: every node of the warp tile has its full family intact and breakable
   const uint32_t *flags32;
   const double *minv;
-  const BTab *btab;                  // [128] exact pass: xi and thr of mask bit q
-  const int *boff;                   // [128] exact pass: cell offset of mask bit q
   const int2 *q8;                    // [128] exact pass: {bit inside the octant words, set of octant words} of mask bit q
+  void *wl;                          // worklist of k_ball_exact: BEntry per warp tile whose filter fired
+  int *wl_count;
   double *v[3];
   const double *bval[3];
   double *theta_out;
   double A, c1, G, vol_uniform, rrho, dt, gramp;   // gramp = g(t_n) = min(1, n dt / ramp_time)
   double xi[3][4];                   // xi[k][a] = a h_k
   double rinv[4][4][4];              // 1 / ||xi||^2 of offset (+-a, +-b, +-c), in the operation order of the walk
+  double thr[4][4][4];               // s_c ||xi||^2 of offset (+-a, +-b, +-c)
+  uint32_t pk[128];                  // mask bit q -> its offset, packed (dx + 3) | (dy + 3) << 4 | (dz + 3) << 8
   int thr_hi[M2 + 1];                // per class |o|^2: min over the class of hi(s_c ||xi||^2)
+  uint32_t cmask[M2 + 1][4];         // per class: its bonds in the four mask words
   alignas(64) CUtensorMap tm_xy, tm_z, tm_g;   // 3-D tiled maps of uxy (as doubles), uz, aux (as doubles)
+};
+
+// worklist entry of a lane whose break filter fired
+template <int RZ>
+struct BEntry {
+  int64_t i0;             // cell of the lane's node at level z0
+  int z0, tile;           // first level; index of the warp tile in tfull
+  uint32_t cm, pad;       // the classes |o|^2 that reached the threshold
+  double acc[RZ];         // per node: sum_j rho_ij dot before the break test
 };
 
 // own-node state of the RZ nodes of a lane (slot l = level z0 + l, or z0 + RZ - 1 - l while sz = -1)
@@ -452,50 +463,23 @@ __global__ void __launch_bounds__(CY * 32, MINB) k_ball(const __grid_constant__ 
   swap_levels<RZ>(p, FORCE);   // the levels back in place
   if constexpr (!FORCE) {
     if constexpr (FRAC) {
-      // ---- break test proper (Eq. 1.30): only where the filter fired ----
-      bool bad = false;
+      uint32_t cm = 0;   // classes |o|^2 whose running max reached the threshold
 #pragma unroll
       for (int c = 1; c <= M2; ++c)
-        if (c != 7) bad = bad || p.mx[c] >= a.thr_hi[c];
-      if (__any_sync(FULL, bad)) {
-        bool broke = false;
+        if (c != 7 && p.mx[c] >= a.thr_hi[c]) cm |= 1u << c;
+      // A lane whose filter fired leaves an entry for k_ball_exact (its nodes, the fired classes, its sums): the walk
+      // never waits for the rare event, and the warps of its CTA are not held up at the plane buffers.
+      const uint32_t fire = __ballot_sync(FULL, cm != 0u);
+      if (fire) {
+        int base = 0;
+        if (lane == 0) base = atomicAdd(a.wl_count, __popc(fire));
+        base = __shfl_sync(FULL, base, 0);
+        if (cm != 0u) {
+          BEntry<RZ> *e = (BEntry<RZ> *)a.wl + base + __popc(fire & ((1u << lane) - 1u));
+          e->i0 = i0; e->z0 = z0; e->tile = (int)(((int64_t)blockIdx.z * a.PY + y0) * a.nxc + xc); e->cm = cm;
 #pragma unroll
-        for (int l = 0; l < RZ; ++l) {
-          if (dead(l)) continue;
-          const int64_t i = cell(l);
-          double acc2 = 0.0;
-#pragma unroll 1
-          for (int w = 0; w < 4; ++w) {
-            uint32_t m = a.mask[(int64_t)w * a.npad + i];
-            const uint32_t nf = a.nofail ? a.nofail[(int64_t)w * a.npad + i] : 0u;
-            const uint32_t m_in = m;
-            uint32_t rem = m;
-            while (rem) {
-              const int bb = __ffs(rem) - 1;
-              rem &= rem - 1u;
-              const int q = w * 32 + bb;
-              const BTab e = a.btab[q];
-              const int64_t j = i + a.boff[q];
-              const double2 xy = a.uxy[j];
-              const double z = a.uz[j];
-              double dot = __dmul_rn(e.xi0, xy.x - p.uo[l][0]);
-              dot = fma(e.xi1, xy.y - p.uo[l][1], dot);
-              dot = fma(e.xi2, z - p.uo[l][2], dot);
-              // s >= s_c breaks: dot >= thr on the bit patterns (thr > 0), identical at both ends of the bond
-              if (__double_as_longlong(dot) >= __double_as_longlong(e.thr) && !((nf >> bb) & 1u)) {
-                m &= ~(1u << bb);
-                const int2 o8 = a.q8[q];   // the bond's copies in the octant words
-                for (int o = 0; o < 8; ++o)
-                  if ((o8.y >> o) & 1) a.mask8[(int64_t)o * a.npad + i] &= ~(1u << o8.x);
-              } else {
-                acc2 += dot;
-              }
-            }
-            if (m != m_in) { a.mask[(int64_t)w * a.npad + i] = m; broke = true; }
-          }
-          p.acc[l] = acc2;
+          for (int l = 0; l < RZ; ++l) e->acc[l] = p.acc[l];
         }
-        if (__any_sync(FULL, broke) && lane == 0) a.tfull[((int64_t)blockIdx.z * a.PY + y0) * a.nxc + xc] = 0;
       }
     }
     double mi[RZ];
@@ -547,6 +531,92 @@ __global__ void __launch_bounds__(CY * 32, MINB) k_ball(const __grid_constant__ 
       a.uxy_w[i] = make_double2(un[0], un[1]);
       a.uz_w[i] = un[2];
     }
+  }
+}
+
+// ---- the break test proper (Eq. 1.30) for the lanes whose filter fired: one warp per entry.  Lane t
+// tests bit t of each mask word of each of the entry's nodes, so all candidate bonds (those of the fired classes) of a
+// node are in flight together: dot >= thr on the bit patterns, bits cleared in the 128-bit masks and in every octant
+// copy, the broken bonds taken out of the sum of Eq. 2.3, theta and {G/m, cth} of the nodes written again.
+template <int RZ>
+__global__ void __launch_bounds__(128, 6) k_ball_exact(const __grid_constant__ BArgs a) {
+  const int lane = threadIdx.x & 31;
+  const int nwarp = (int)((gridDim.x * blockDim.x) >> 5), count = *a.wl_count;
+  const int64_t zstr = (int64_t)a.DY * a.DX;
+  for (int en = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5); en < count; en += nwarp) {
+    const BEntry<RZ> *e = (const BEntry<RZ> *)a.wl + en;
+    const int64_t i0 = e->i0;
+    const int z0 = e->z0;
+    const uint32_t cm = e->cm;
+    uint32_t cand[4] = {0u, 0u, 0u, 0u};   // the bonds of the fired classes, per mask word
+    for (int c = 1; c <= M2; ++c)
+      if ((cm >> c) & 1u) {
+#pragma unroll
+        for (int w = 0; w < 4; ++w) cand[w] |= a.cmask[c][w];
+      }
+    bool broke = false;
+#pragma unroll
+    for (int l = 0; l < RZ; ++l) {
+      if (z0 + l >= a.PZ) continue;   // dead
+      const int64_t i = i0 + l * zstr;
+      const double2 uxy = a.uxy[i];
+      const double u0 = uxy.x, u1 = uxy.y, u2 = a.uz[i];
+      uint32_t m[4];
+      bool has[4];
+      double x0[4], x1[4], x2[4], thr[4];
+      double2 xy[4];
+      double z[4];
+#pragma unroll
+      for (int w = 0; w < 4; ++w) {   // this lane's candidate of each word: offset and geometry from the packed table
+        m[w] = a.mask[(int64_t)w * a.npad + i];
+        const uint32_t nf = a.nofail ? a.nofail[(int64_t)w * a.npad + i] : 0u;
+        has[w] = ((m[w] & ~nf & cand[w]) >> lane) & 1u;
+        const uint32_t pk = a.pk[w * 32 + lane];
+        const int dx = (int)(pk & 15u) - S, dy = (int)((pk >> 4) & 15u) - S, dz = (int)((pk >> 8) & 15u) - S;
+        x0[w] = signed_const(a.xi[0][abs(dx)], dx < 0 ? (int)0x80000000 : 0);
+        x1[w] = signed_const(a.xi[1][abs(dy)], dy < 0 ? (int)0x80000000 : 0);
+        x2[w] = signed_const(a.xi[2][abs(dz)], dz < 0 ? (int)0x80000000 : 0);
+        thr[w] = a.thr[abs(dx)][abs(dy)][abs(dz)];
+        const int64_t j = has[w] ? i + ((int64_t)dz * a.DY + dy) * a.DX + dx : i;
+        xy[w] = a.uxy[j];
+        z[w] = a.uz[j];
+      }
+      double sub = 0.0;
+      bool brokel = false;
+#pragma unroll
+      for (int w = 0; w < 4; ++w) {
+        // the dot of the walk, bit for bit (a vanishing component of xi adds an exact zero)
+        double dot = __dmul_rn(x0[w], xy[w].x - u0);
+        dot = fma(x1[w], xy[w].y - u1, dot);
+        dot = fma(x2[w], z[w] - u2, dot);
+        // s >= s_c breaks: dot >= thr on the bit patterns (thr > 0), identical at both ends of the bond
+        const bool brk = has[w] && __double_as_longlong(dot) >= __double_as_longlong(thr[w]);
+        const uint32_t bb = __ballot_sync(FULL, brk);
+        if (bb) {
+          if (brk) {   // the bond's copies in the octant words (several lanes may share a word)
+            const int2 o8 = a.q8[w * 32 + lane];
+            for (int o = 0; o < 8; ++o)
+              if ((o8.y >> o) & 1) atomicAnd(&a.mask8[(int64_t)o * a.npad + i], ~(1u << o8.x));
+          }
+          if (lane == 0) a.mask[(int64_t)w * a.npad + i] = m[w] & ~bb;
+          double d = brk ? dot : 0.0;   // rho_ij <- 0: the bonds leave the sum of Eq. 2.3 (fixed summation order)
+#pragma unroll
+          for (int off = 16; off; off >>= 1) d += __shfl_xor_sync(FULL, d, off);
+          sub += d;
+          brokel = true;
+        }
+      }
+      if (brokel) {
+        broke = true;
+        if (lane == 0) {
+          const double mi = a.minv[i];
+          const double theta = a.A * mi * ((e->acc[l] - sub) * a.vol_uniform);   // as in the epilogue of the walk
+          a.aux[i] = make_double2(a.G * mi, a.c1 * theta * mi);
+          if (a.theta_out) a.theta_out[i] = theta;
+        }
+      }
+    }
+    if (broke && lane == 0) a.tfull[e->tile] = 0;
   }
 }
 
@@ -645,20 +715,12 @@ void ball_launch(const BPrepared *pp, cudaStream_t st) {
 bool ball_tables(pd_sim *s) {
   PdLattice &l = s->lat;
   if (l.ball_q8) return true;
-  std::vector<BTab> tab(128, BTab{0.0, 0.0, 0.0, 0.0});
-  std::vector<int> off(128, 0);
   std::vector<int2> q8(128, make_int2(0, 0));
   for (int dz = -S; dz <= S; ++dz)
     for (int dy = -S; dy <= S; ++dy)
       for (int dx = -S; dx <= S; ++dx) {
         if (!inball(dx, dy, dz)) continue;
         const int b = ball_bit(dx, dy, dz);
-        const double x0 = (double)dx * l.h[0], x1 = (double)dy * l.h[1], x2 = (double)dz * l.h[2];
-        double r2 = x0 * x0;
-        r2 = std::fma(x1, x1, r2);
-        r2 = std::fma(x2, x2, r2);
-        tab[b] = BTab{x0, x1, x2, s->s_c * r2};
-        off[b] = (dz * l.DY + dy) * l.DX + dx;
         int octs = 0;
         for (int o = 0; o < 8; ++o) {
           const int sx = o & 1, sy = (o >> 1) & 1, sz = (o >> 2) & 1;
@@ -667,15 +729,11 @@ bool ball_tables(pd_sim *s) {
         }
         q8[b] = make_int2(canon(abs(dx), abs(dy), abs(dz)), octs);
       }
-  BTab *tab_d = (BTab *)pdi::dev_alloc(s, sizeof(BTab) * 128);
-  int *off_d = (int *)pdi::dev_alloc(s, sizeof(int) * 128);
   int2 *q8_d = (int2 *)pdi::dev_alloc(s, sizeof(int2) * 128);
   uint32_t *m8 = (uint32_t *)pdi::dev_alloc(s, sizeof(uint32_t) * 8 * s->npad);
   uint32_t *n8 = l.nofail ? (uint32_t *)pdi::dev_alloc(s, sizeof(uint32_t) * 8 * s->npad) : nullptr;
-  if (!tab_d || !off_d || !q8_d || !m8 || (l.nofail && !n8)) return false;
-  if (cudaMemcpyAsync(tab_d, tab.data(), sizeof(BTab) * 128, cudaMemcpyHostToDevice, s->stream) != cudaSuccess ||
-      cudaMemcpyAsync(off_d, off.data(), sizeof(int) * 128, cudaMemcpyHostToDevice, s->stream) != cudaSuccess ||
-      cudaMemcpyAsync(q8_d, q8.data(), sizeof(int2) * 128, cudaMemcpyHostToDevice, s->stream) != cudaSuccess) {
+  if (!q8_d || !m8 || (l.nofail && !n8)) return false;
+  if (cudaMemcpyAsync(q8_d, q8.data(), sizeof(int2) * 128, cudaMemcpyHostToDevice, s->stream) != cudaSuccess) {
     cudaGetLastError();
     return false;
   }
@@ -683,7 +741,7 @@ bool ball_tables(pd_sim *s) {
   k_ball_octants<<<nblk, 256, 0, s->stream>>>(s->npad, l.nbits, q8_d, l.mask, m8);
   if (n8) k_ball_octants<<<nblk, 256, 0, s->stream>>>(s->npad, l.nbits, q8_d, l.nofail, n8);
   if (cudaGetLastError() != cudaSuccess || cudaStreamSynchronize(s->stream) != cudaSuccess) { cudaGetLastError(); return false; }
-  l.ball_btab = tab_d; l.ball_boff = off_d; l.ball_q8 = q8_d; l.mask8 = m8; l.nf8 = n8;
+  l.ball_q8 = q8_d; l.mask8 = m8; l.nf8 = n8;
   return true;
 }
 
@@ -717,10 +775,19 @@ BPrepared *ball_prepare(pd_sim *s, bool force) {
     return r2;
   };
   for (int c = 0; c <= M2; ++c) a.thr_hi[c] = 0x7ff00000;
+  for (int q = 0; q < 128; ++q) a.pk[q] = (uint32_t)S | (uint32_t)S << 4 | (uint32_t)S << 8;   // (unused bits: the zero offset)
+  for (int dz = -S; dz <= S; ++dz)
+    for (int dy = -S; dy <= S; ++dy)
+      for (int dx = -S; dx <= S; ++dx)
+        if (inball(dx, dy, dz)) {
+          a.cmask[dx * dx + dy * dy + dz * dz][ball_bit(dx, dy, dz) >> 5] |= 1u << (ball_bit(dx, dy, dz) & 31);
+          a.pk[ball_bit(dx, dy, dz)] = (uint32_t)(dx + S) | (uint32_t)(dy + S) << 4 | (uint32_t)(dz + S) << 8;
+        }
   for (int i = 0; i < 4; ++i)
     for (int j = 0; j < 4; ++j)
       for (int k = 0; k < 4; ++k) {
         a.rinv[i][j][k] = (i | j | k) ? 1.0 / r2of(i, j, k) : 0.0;
+        a.thr[i][j][k] = s->s_c * r2of(i, j, k);
         if (!inball(i, j, k)) continue;
         const double thr = s->s_c * r2of(i, j, k);
         long long bits;
@@ -728,7 +795,7 @@ BPrepared *ball_prepare(pd_sim *s, bool force) {
         a.thr_hi[i * i + j * j + k * k] = std::min(a.thr_hi[i * i + j * j + k * k], (int)(bits >> 32));
       }
   if (!ball_tables(s)) return pp;
-  a.btab = (const BTab *)l.ball_btab; a.boff = (const int *)l.ball_boff; a.q8 = (const int2 *)l.ball_q8;
+  a.q8 = (const int2 *)l.ball_q8;
   a.mask8 = l.mask8; a.nf8 = l.nf8;
   if (!l.ball_tfull) {   // the warp-tile flags (kept in step by the exact pass)
     const int ntiles = ((l.PZ + BRZ - 1) / BRZ) * l.PY * a.nxc;
@@ -740,6 +807,14 @@ BPrepared *ball_prepare(pd_sim *s, bool force) {
     l.ball_tfull = tf;
   }
   a.tfull = l.ball_tfull;
+  if (!l.ball_wl && s->fracture) {   // worklist of the break test: at most one entry per lane and launch
+    const size_t ntiles = (size_t)((l.PZ + BRZ - 1) / BRZ) * l.PY * a.nxc;
+    void *wl = pdi::dev_alloc(s, ntiles * 32 * sizeof(BEntry<BRZ>));
+    int *cnt = (int *)pdi::dev_alloc(s, sizeof(int));
+    if (!wl || !cnt) return pp;
+    l.ball_wl = wl; l.ball_wl_count = cnt;
+  }
+  a.wl = l.ball_wl; a.wl_count = l.ball_wl_count;
   const int sy = pp->cy + 2 * S;
   bool ok = true;
   for (int q = 0; q < 2 && ok; ++q)
@@ -773,7 +848,13 @@ int ball_launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
   a.uxy = l.uxy[s->cur]; a.uz = l.uz[s->cur]; a.uxy_w = nullptr; a.uz_w = nullptr;
   a.tm_xy = pp->tm_xy[s->cur]; a.tm_z = pp->tm_z[s->cur]; a.tm_g = pp->tm_g;
   a.theta_out = theta_out;
-  if (do_break && s->fracture) ball_launch<false, true>(pp, s->stream); else ball_launch<false, false>(pp, s->stream);
+  if (do_break && s->fracture) {
+    if (cudaMemsetAsync(a.wl_count, 0, sizeof(int), s->stream) != cudaSuccess) { cudaGetLastError(); return 0; }
+    ball_launch<false, true>(pp, s->stream);
+    k_ball_exact<BRZ><<<148 * 6, 128, 0, s->stream>>>(a);   // (exits at once while no filter fires)
+  } else {
+    ball_launch<false, false>(pp, s->stream);
+  }
   return 1;
 }
 
