@@ -534,17 +534,18 @@ __global__ void __launch_bounds__(CY * 32, MINB) k_ball(const __grid_constant__ 
   }
 }
 
-// ---- the break test proper (Eq. 1.30) for the lanes whose filter fired: one warp per entry.  Lane t
-// tests bit t of each mask word of each of the entry's nodes, so all candidate bonds (those of the fired classes) of a
-// node are in flight together: dot >= thr on the bit patterns, bits cleared in the 128-bit masks and in every octant
+// ---- the break test proper (Eq. 1.30) for the lanes whose filter fired: one warp per entry and node.
+// Lane t tests bit t of each mask word of the node, so all its candidate bonds (those of the fired classes) are in
+// flight together: dot >= thr on the bit patterns, bits cleared in the 128-bit masks and in every octant
 // copy, the broken bonds taken out of the sum of Eq. 2.3, theta and {G/m, cth} of the nodes written again.
 template <int RZ>
 __global__ void __launch_bounds__(128, 6) k_ball_exact(const __grid_constant__ BArgs a) {
   const int lane = threadIdx.x & 31;
   const int nwarp = (int)((gridDim.x * blockDim.x) >> 5), count = *a.wl_count;
   const int64_t zstr = (int64_t)a.DY * a.DX;
-  for (int en = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5); en < count; en += nwarp) {
-    const BEntry<RZ> *e = (const BEntry<RZ> *)a.wl + en;
+  for (int task = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5); task < count * RZ; task += nwarp) {
+    const BEntry<RZ> *e = (const BEntry<RZ> *)a.wl + task / RZ;
+    const int l = task % RZ;
     const int64_t i0 = e->i0;
     const int z0 = e->z0;
     const uint32_t cm = e->cm;
@@ -554,9 +555,7 @@ __global__ void __launch_bounds__(128, 6) k_ball_exact(const __grid_constant__ B
 #pragma unroll
         for (int w = 0; w < 4; ++w) cand[w] |= a.cmask[c][w];
       }
-    bool broke = false;
-#pragma unroll
-    for (int l = 0; l < RZ; ++l) {
+    {
       if (z0 + l >= a.PZ) continue;   // dead
       const int64_t i = i0 + l * zstr;
       const double2 uxy = a.uxy[i];
@@ -606,17 +605,14 @@ __global__ void __launch_bounds__(128, 6) k_ball_exact(const __grid_constant__ B
           brokel = true;
         }
       }
-      if (brokel) {
-        broke = true;
-        if (lane == 0) {
-          const double mi = a.minv[i];
-          const double theta = a.A * mi * ((e->acc[l] - sub) * a.vol_uniform);   // as in the epilogue of the walk
-          a.aux[i] = make_double2(a.G * mi, a.c1 * theta * mi);
-          if (a.theta_out) a.theta_out[i] = theta;
-        }
+      if (brokel && lane == 0) {
+        const double mi = a.minv[i];
+        const double theta = a.A * mi * ((e->acc[l] - sub) * a.vol_uniform);   // as in the epilogue of the walk
+        a.aux[i] = make_double2(a.G * mi, a.c1 * theta * mi);
+        if (a.theta_out) a.theta_out[i] = theta;
+        a.tfull[e->tile] = 0;
       }
     }
-    if (broke && lane == 0) a.tfull[e->tile] = 0;
   }
 }
 
@@ -851,7 +847,7 @@ int ball_launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
   if (do_break && s->fracture) {
     if (cudaMemsetAsync(a.wl_count, 0, sizeof(int), s->stream) != cudaSuccess) { cudaGetLastError(); return 0; }
     ball_launch<false, true>(pp, s->stream);
-    k_ball_exact<BRZ><<<148 * 6, 128, 0, s->stream>>>(a);   // (exits at once while no filter fires)
+    k_ball_exact<BRZ><<<148 * 12, 128, 0, s->stream>>>(a);   // (exits at once while no filter fires)
   } else {
     ball_launch<false, false>(pp, s->stream);
   }
