@@ -58,7 +58,7 @@ def byte_model(n, z, dim, fracture):
 
 # FP64 instructions the arithmetic of the shipped kernels needs per directed bond (dilatation, force), by layout
 # (counted in the SASS of the FAST step: profiles/r02_kernels.md)
-FP64_PER_BOND = {2: (7.0, 12.5), 1: (10.0, 22.0), 0: (10.0, 22.0)}
+FP64_PER_BOND = {3: (686.0 / 122.0, 1334.0 / 122.0), 2: (7.0, 12.5), 1: (10.0, 22.0), 0: (10.0, 22.0)}
 
 
 def kernel_source_hash():

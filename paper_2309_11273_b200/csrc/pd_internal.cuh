@@ -219,6 +219,7 @@ void ulat_free_cache(pd_sim *s);
 int ball_launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
 int ball_launch_force_update(pd_sim *s);
 void ball_free_cache(pd_sim *s);
+bool ball_eligible(const pd_sim *s);
 // pd_step.cu
 int launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
 int launch_force_update(pd_sim *s);

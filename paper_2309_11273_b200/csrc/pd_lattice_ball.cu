@@ -542,7 +542,23 @@ template <int RZ>
 __global__ void __launch_bounds__(128, 6) k_ball_exact(const __grid_constant__ BArgs a) {
   const int lane = threadIdx.x & 31;
   const int nwarp = (int)((gridDim.x * blockDim.x) >> 5), count = *a.wl_count;
+  if (count == 0) return;
   const int64_t zstr = (int64_t)a.DY * a.DX;
+  // per mask bit q: xi, thr and the cell offset, in shared memory (thread q fills entry q: a lane-dependent index into the
+  // constant bank is serialised, so it is paid once per CTA, not per candidate bond)
+  __shared__ double tx0[128], tx1[128], tx2[128], tthr[128];
+  __shared__ int64_t toff[128];
+  {
+    const int q = threadIdx.x;
+    const uint32_t pk = a.pk[q];
+    const int dx = (int)(pk & 15u) - S, dy = (int)((pk >> 4) & 15u) - S, dz = (int)((pk >> 8) & 15u) - S;
+    tx0[q] = signed_const(a.xi[0][abs(dx)], dx < 0 ? (int)0x80000000 : 0);
+    tx1[q] = signed_const(a.xi[1][abs(dy)], dy < 0 ? (int)0x80000000 : 0);
+    tx2[q] = signed_const(a.xi[2][abs(dz)], dz < 0 ? (int)0x80000000 : 0);
+    tthr[q] = a.thr[abs(dx)][abs(dy)][abs(dz)];
+    toff[q] = ((int64_t)dz * a.DY + dy) * a.DX + dx;
+  }
+  __syncthreads();
   for (int task = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5); task < count * RZ; task += nwarp) {
     const BEntry<RZ> *e = (const BEntry<RZ> *)a.wl + task / RZ;
     const int l = task % RZ;
@@ -570,13 +586,9 @@ __global__ void __launch_bounds__(128, 6) k_ball_exact(const __grid_constant__ B
         m[w] = a.mask[(int64_t)w * a.npad + i];
         const uint32_t nf = a.nofail ? a.nofail[(int64_t)w * a.npad + i] : 0u;
         has[w] = ((m[w] & ~nf & cand[w]) >> lane) & 1u;
-        const uint32_t pk = a.pk[w * 32 + lane];
-        const int dx = (int)(pk & 15u) - S, dy = (int)((pk >> 4) & 15u) - S, dz = (int)((pk >> 8) & 15u) - S;
-        x0[w] = signed_const(a.xi[0][abs(dx)], dx < 0 ? (int)0x80000000 : 0);
-        x1[w] = signed_const(a.xi[1][abs(dy)], dy < 0 ? (int)0x80000000 : 0);
-        x2[w] = signed_const(a.xi[2][abs(dz)], dz < 0 ? (int)0x80000000 : 0);
-        thr[w] = a.thr[abs(dx)][abs(dy)][abs(dz)];
-        const int64_t j = has[w] ? i + ((int64_t)dz * a.DY + dy) * a.DX + dx : i;
+        const int q = w * 32 + lane;
+        x0[w] = tx0[q]; x1[w] = tx1[q]; x2[w] = tx2[q]; thr[w] = tthr[q];
+        const int64_t j = has[w] ? i + toff[q] : i;
         xy[w] = a.uxy[j];
         z[w] = a.uz[j];
       }
@@ -828,6 +840,9 @@ BPrepared *ball_prepare(pd_sim *s, bool force) {
 
 namespace pdi {
 
+// does this handle take the kernels of this file?  (the layout pd_get_layout reports)
+bool ball_eligible(const pd_sim *s) { return env_int("PD_BALL", 1) != 0 && ball_layout_matches(s); }
+
 void ball_free_cache(pd_sim *s) {
   for (int q = 4; q < 6; ++q) {
     delete (BPrepared *)s->lat.cache[q];
@@ -848,6 +863,7 @@ int ball_launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
     if (cudaMemsetAsync(a.wl_count, 0, sizeof(int), s->stream) != cudaSuccess) { cudaGetLastError(); return 0; }
     ball_launch<false, true>(pp, s->stream);
     k_ball_exact<BRZ><<<148 * 12, 128, 0, s->stream>>>(a);   // (exits at once while no filter fires)
+    s->launches += 1;
   } else {
     ball_launch<false, false>(pp, s->stream);
   }

@@ -82,7 +82,7 @@ def test_config5p_full_breaking():
     from paper_2309_11273_b200 import workloads as W
     wl = W.cylinder3d(l_cells=160, omega=400.0)
     sim, o = _sim(wl), _oracle(wl)
-    assert sim.get_layout()["layout"] == 2 and wl.n == 1257600
+    assert sim.get_layout()["layout"] == 3 and wl.n == 1257600   # the compiled-in 122-offset stencil kernels
     nsteps = 300
     sim.step(nsteps); o.step(nsteps)
     bs, ob = _broken_set(sim), o.broken_set()

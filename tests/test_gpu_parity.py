@@ -13,8 +13,9 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-10
 
 # the code paths of the library: the layout is chosen inside pd_create; the environment
-# switches exist for exactly this purpose (and for profiling).  Layout codes (pd_get_layout): 2 = uniform
-# lattice (constant bond geometry per stencil offset; the default on the unjittered grids of configs 1, 2, 3, 5),
+# switches exist for exactly this purpose (and for profiling).  Layout codes (pd_get_layout): 3 = uniform lattice with
+# the compiled-in 122-offset stencil (3-D, horizon 3.015 dx: config 5), 2 = uniform
+# lattice (constant bond geometry per stencil offset; the default on the unjittered grids of configs 1, 2, 3),
 # 1 = dense lattice with per-bond geometry (jittered config 4; PD_LAT_UNIFORM=0 forces it), 0 = sliced ELL.
 LAYOUTS = {
     "default": ({}, None),
@@ -50,7 +51,10 @@ def _expect_layout(code, wl):
     """the layout pd_create must pick by itself: jittered lattices cannot take the uniform path"""
     if code is not None:
         return code
-    return 1 if wl.name == "block3d" and wl.meta.get("jitter", 1.0) != 0.0 else 2
+    if wl.name == "block3d" and wl.meta.get("jitter", 1.0) != 0.0:
+        return 1
+    import os
+    return 3 if wl.dim == 3 and os.environ.get("PD_BALL", "1") != "0" else 2   # 3: the compiled-in 122-offset stencil
 
 
 def _oracle(wl):
@@ -286,7 +290,7 @@ def test_full_size_config5p_sampled():
     from paper_2309_11273_b200 import workloads as W
     wl = W.CONFIGS["config5p"]()
     sim, o = _sim(wl), _oracle(wl)
-    assert sim.get_layout()["layout"] == 2
+    assert sim.get_layout()["layout"] == 3   # the compiled-in 122-offset stencil kernels
     assert sim.get_stats()["n_directed_bonds"] == o.Z
     sim.step(3); o.step(3)
     assert _rel(sim.get_u(), o.u) <= TOL and _rel(sim.get_v(), o.v) <= TOL
