@@ -29,12 +29,14 @@ LAYOUTS = {
                      "PD_ULAT_FRC_CY": "2", "PD_BALL": "0"}, None),
     # table-driven staged kernels with their default shape
     "uniform_table": ({"PD_BALL": "0"}, None),
+    # compiled-in stencil kernels in their other launch shape: 4 rows per CTA, 3 plane buffers in flight
+    "ball_cy4_nb3": ({"PD_BALL_CY": "4", "PD_BALL_NB": "3"}, None),
     "lattice_general": ({"PD_LAT_UNIFORM": "0"}, 1),
     "lattice_general_2rows": ({"PD_LAT_UNIFORM": "0", "PD_DIR_DIL_ROWS": "2", "PD_DIR_FRC_ROWS": "2"}, 1),
     "sliced_ell": ({"PD_FORCE_GENERIC": "1"}, 0),
 }
 _ENV_KEYS = ("PD_LAT_UNIFORM", "PD_FORCE_GENERIC", "PD_DIR_DIL_ROWS", "PD_DIR_FRC_ROWS", "PD_ULAT_DIL_ROWS",
-             "PD_ULAT_FRC_ROWS", "PD_ULAT_STAGED", "PD_ULAT_NB", "PD_ULAT_DIL_CY", "PD_ULAT_FRC_CY", "PD_GRAPH", "PD_BALL")
+             "PD_ULAT_FRC_ROWS", "PD_ULAT_STAGED", "PD_ULAT_NB", "PD_ULAT_DIL_CY", "PD_ULAT_FRC_CY", "PD_GRAPH", "PD_BALL", "PD_BALL_CY", "PD_BALL_NB")
 
 
 @pytest.fixture(params=list(LAYOUTS))
