@@ -347,11 +347,12 @@ static int graph_build(pd_sim *s, int which, int nsteps) {
   for (int it = 0; it < nsteps && rc == PD_OK; ++it) rc = step_once(s);
   if (cudaStreamEndCapture(s->cap_stream, &g) != cudaSuccess) rc = rc ? rc : PD_ERR_CUDA;
   s->stream = user;
+  const int64_t captured = s->launches - launches0;
   s->cur = cur0; s->step = step0; s->launches = launches0;   // nothing ran
   if (rc == PD_OK && cudaGraphInstantiate(&s->graph[which], g, 0) != cudaSuccess) rc = PD_ERR_CUDA;
   if (g) cudaGraphDestroy(g);
   if (rc != PD_OK) { cudaGetLastError(); s->graph[which] = nullptr; }
-  else s->graph_steps[which] = nsteps;
+  else { s->graph_steps[which] = nsteps; s->graph_launches[which] = captured; }
   return rc;
 }
 
@@ -376,7 +377,7 @@ int pd_step(pd_sim *s, int64_t nsteps) {
       }
       if (s->graph[which]) {
         PD_CUDA(cudaGraphLaunch(s->graph[which], s->stream));
-        s->step += len; s->launches += 2 * len;   // cur is back at 0 after an even number of steps
+        s->step += len; s->launches += s->graph_launches[which];   // cur is back at 0 after an even number of steps
         left -= len;
         continue;
       }

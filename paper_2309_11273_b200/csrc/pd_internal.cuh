@@ -183,6 +183,7 @@ struct pd_sim {
   bool use_graph = true, graph_failed = false;
   int graph_len = 32;
   int graph_steps[2] = {0, 0};
+  int64_t graph_launches[2] = {0, 0};   // kernels inside one replay of the graph
   cudaGraphExec_t graph[2] = {nullptr, nullptr};
   cudaStream_t cap_stream = nullptr;
   unsigned long long *stats_dev = nullptr;  // [0]=broken directed, [1]=max phi bits, [2]=#phi>=.5

@@ -144,6 +144,46 @@ def test_fracture_broken_sets(name, layout):
     sim.destroy()
 
 
+@pytest.mark.parametrize("fracture", [False, True])
+def test_uniform_block_traction_ramp_and_mixed_dofs(fracture):
+    """Eq. 2.11 with the ramped body force g(t_n) b and per-dof boundary flags (App. B; C-3, C-4, C-14)
+    on the compiled-in stencil kernels of a plain 3-D lattice: traction on the far face ramped over 40 steps, the near
+    face clamped in x only, one edge with a prescribed z velocity; with and without the break filter / break test
+    (s_c chosen so that the loaded face tears off within the run)."""
+    from paper_2309_11273_b200 import workloads as W
+    wl = W.block3d(nx=70, ny=13, nz=11, jitter=0.0)
+    ix = np.rint(wl.coords[:, 0] / wl.dx - 0.5).astype(int)
+    iy = np.rint(wl.coords[:, 1] / wl.dx - 0.5).astype(int)
+    wl.u0[:] = 0.0
+    wl.flags[:] = 0
+    wl.value[:] = 0.0
+    wl.flags[ix < 3] = W.CLAMP_X
+    far = ix >= 69
+    wl.flags[far] = W.BODY_FORCE
+    wl.value[far, 0] = 4.0e6 / wl.dx            # sigma / dx on the outermost node layer (C-14)
+    wl.value[far, 1] = -1.0e6 / wl.dx
+    edge = (ix >= 30) & (ix < 40) & (iy == 0)
+    wl.flags[edge] |= W.PRESC_Z
+    wl.value[edge, 2] = 0.05
+    wl.ramp_time = 40 * wl.dt
+    if fracture:
+        wl.s_c = 2.0e-5
+    sim, o = _sim(wl), _oracle(wl)
+    assert sim.get_layout()["layout"] == 3
+    nsteps, total = 120, 0
+    for chunk in (1, 39, 80):
+        sim.step(chunk)
+        total += o.step(chunk)
+        if fracture:
+            bs, _, _ = _broken_set(sim)
+            assert o.near_total == 0 and bs == o.broken_set()
+        assert _rel(sim.get_u(), o.u) <= (1e-9 if fracture else TOL)
+        assert _rel(sim.get_v(), o.v) <= (1e-9 if fracture else TOL)
+    assert (total > 0) == fracture
+    assert sim.get_stats()["step"] == nsteps
+    sim.destroy()
+
+
 def test_nonuniform_volume_and_device_pointers():
     """general path: non-uniform V, inputs/outputs as torch CUDA tensors, library allocator."""
     import torch
