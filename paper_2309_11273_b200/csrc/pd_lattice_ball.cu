@@ -293,7 +293,9 @@ __device__ __forceinline__ void swap_levels(ST &p, bool force) {
 template <bool FORCE, bool FRAC, int RZ, int CY, int NB, int MINB>
 __global__ void __launch_bounds__(CY * 32, MINB) k_ball(const __grid_constant__ BArgs a) {
   using SM = BSmem<FORCE, FRAC, RZ, CY, NB>;
-  constexpr int NP = RZ + 2 * S, NT = CY * 32;
+  // planes z0 - S + 1 .. z0 + RZ + S - 2: the two outermost planes of the stencil would each serve ONE bond of the lane
+  // (offset (0, 0, -+S) of its first / last node), which is read from global memory instead
+  constexpr int NP = RZ + 2 * S - 2, NT = CY * 32;
   constexpr bool BRK = !FORCE && FRAC;
   static_assert(RZ % 2 == 0, "the mirrored walk needs an even number of levels per lane");
   extern __shared__ __align__(128) unsigned char smraw[];
@@ -316,13 +318,13 @@ __global__ void __launch_bounds__(CY * 32, MINB) k_ball(const __grid_constant__ 
   }
   if (!__syncthreads_or(active)) return;   // barriers visible; nothing to do for the whole CTA?
   // the planes are consumed in the order NP/2 - 1 .. 0, NP/2 .. NP - 1 (the planes with most bonds first in each half,
-  // so their walk hides the next loads); position k of that order holds the box
+  // so their walk hides the next loads; plane q is level z0 - S + 1 + q); position k of that order holds the box
   // [xc 32 + HX - S, +BSX) x [yt + HY - S, +sy) of level z0 + HZ - S + plane(k)
   auto issue = [&](int k) {
     const int b = k % NB;
     unsigned char *dst = smraw + SM::o_buf + b * SM::plane;
     const int plane = k < NP / 2 ? NP / 2 - 1 - k : k;
-    const int cx = xc * 32 + a.HX - S, cyy = blockIdx.y * CY + a.HY - S, czz = z0 + a.HZ - S + plane;
+    const int cx = xc * 32 + a.HX - S, cyy = blockIdx.y * CY + a.HY - S, czz = z0 + a.HZ - S + 1 + plane;
     mbar_expect_tx(&full[b], SM::tx);
     tma_load_3d(dst, &a.tm_xy, 2 * cx, cyy, czz, &full[b]);
     tma_load_3d(dst + SM::o_z, &a.tm_z, cx, cyy, czz, &full[b]);
@@ -416,8 +418,18 @@ __global__ void __launch_bounds__(CY * 32, MINB) k_ball(const __grid_constant__ 
 #pragma unroll
       for (int c = 1; c < 4; ++c) { sg.xs2[c] = signed_const(a.xi[2][c], mz << 31); keep(sg.xs2[c]); }
     }
+    // the record three levels beyond the lane's first node (its last node while sz = -1): on its way during the planes
+    double2 fxy = make_double2(0.0, 0.0), fg = make_double2(0.0, 0.0);
+    double fz = 0.0;
+    if (active) {
+      const int nl = mz ? RZ - 1 : 0;
+      const int64_t j = dead(nl) ? i0 : cell(nl) + (mz ? S : -S) * zstr;
+      fxy = a.uxy[j];
+      fz = a.uz[j];
+      if constexpr (FORCE) fg = a.aux[j];
+    }
     sfor<0, NP / 2>([&](auto Jc) {
-      constexpr int J = NP / 2 - 1 - CV(Jc);   // plane J of the first half, or its mirror image NP - 1 - J
+      constexpr int J = NP / 2 - CV(Jc);   // plane of the stencil (pz = J - S relative to slot 0), or its mirror image
       const int k = mz * (NP / 2) + CV(Jc), b = k % NB;
       if (k > 0) leave(k);
       mbar_wait(&full[b], (k / NB) & 1);
@@ -458,6 +470,16 @@ __global__ void __launch_bounds__(CY * 32, MINB) k_ball(const __grid_constant__ 
         }
       }
     });
+    if (active) {   // offset (0, 0, -S) of slot 0
+      if (fast) {
+        ball_bond<FORCE, FRAC, false, 0, 0, -S, 0>(a, p, sg, fxy, fz, fg);
+      } else {
+        const int nl = mz ? RZ - 1 : 0, on = 4 * (mz ^ 1) * RZ;
+        p.wneg[0] = m8s[(on + nl) * NT];
+        if constexpr (BRK) p.bneg[0] = b8s[(on + nl) * NT];
+        ball_bond<FORCE, FRAC, true, 0, 0, -S, 0>(a, p, sg, fxy, fz, fg);
+      }
+    }
   }
   if (!active) return;
   swap_levels<RZ>(p, FORCE);   // the levels back in place
