@@ -8,16 +8,18 @@
 //        theta_i = (A / m_i) V sum_j rho_ij dot  (Eq. 1.6 / 2.3)
 //        s >= s_c  <=>  dot >= thr = s_c ||xi||^2 (Eqs. 1.17, 1.30).  The walk only FILTERS:
 //        per class |o|^2 a running integer max of the high words of dot against the high word of the smallest thr of
-//        the class (hi(dot) < hi(thr) => dot < thr).  A warp whose filter fires runs the EXACT pass at the end: bond by
-//        bond from global memory, dot >= thr on the bit patterns, bits cleared, theta re-summed without them.  Both
-//        ends of a bond compute the same dot bit for bit (negating xi and eta is exact), so they decide alike (C-6).
+//        the class (hi(dot) < hi(thr) => dot < thr).  A lane whose filter fires leaves a worklist entry; k_ball_exact,
+//        launched after the pass, tests the bonds of the fired classes with dot >= thr on the bit patterns, clears the
+//        bits and takes the broken bonds out of theta (the walk never waits for the rare event).  Both ends of a bond
+//        compute the same dot bit for bit (negating xi and eta is exact), so they decide alike (C-6).
 //   force:  d = dot / ||xi||^2,  t = (cth_i + cth_j) + (G/m_i + G/m_j) d,  f_i += t xi          7 / 10 / 13 FP64
 //        (Eq. 2.2 / 2.1), then Eq. 2.11 and the boundary dofs of App. B in the epilogue.
 //
 // Kernel shape: lanes along x, a lane owns RZ nodes adjacent in z (one row), so a gathered record serves up to RZ bonds
 // from registers (0.43 shared-memory records per bond at RZ = 4); a CTA is CY warps adjacent in y and consumes the
-// RZ + 6 planes z0 - 3 .. z0 + RZ + 2, each brought into shared memory once by TMA (NB buffers in flight, completion on
-// an mbarrier, a buffer handed back by the last warp that leaves it: no CTA barrier).
+// RZ + 4 planes z0 - 2 .. z0 + RZ + 1, each brought into shared memory once by TMA (NB buffers in flight, completion on
+// an mbarrier, a buffer handed back by the last warp that leaves it: no CTA barrier); the two outermost planes of the
+// stencil serve one bond per lane each, and that record is read from global memory instead.
 //
 // The MIRRORED walk.  Unrolling all 122 RZ bonds of a lane gives 8-17 k instructions, which do not fit the instruction
 // cache: that version ran at one instruction per clock and SM (profiles/r02b_ball_kernels.md, stall_no_instruction 7-8
@@ -32,7 +34,7 @@
 // the bond bit of offset (sx a, sy b, sz c) at a compile-time position: the OCTANT words mask8[oct][cell], oct = the
 // three sign bits, bit = index of (a, b, c) among the 28 magnitudes (an offset with a zero component sits in both
 // words of that sign).  They are derived from the 128-bit masks of the lattice layout (which stay the truth for every
-// other kernel) when the kernels are prepared and are kept in step by the exact pass.
+// other kernel) when the kernels are prepared and are kept in step by k_ball_exact.
 //
 // Taken only when the lattice's stencil and mask-bit layout are exactly the ball's (checked in ball_prepare);
 // every other uniform lattice takes the table-driven kernels of pd_lattice_uniform.cu.
