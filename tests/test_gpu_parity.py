@@ -144,6 +144,24 @@ def test_fracture_broken_sets(name, layout):
     sim.destroy()
 
 
+def test_compiled_in_stencil_run_to_run_reproducible():
+    """The break test of the compiled-in stencil kernels goes through a worklist filled with atomics (entry order varies
+    from run to run) and clears octant-word bits with atomics: the state must not depend on that order.  Two runs of the
+    long cylinder, bonds breaking, must agree bit for bit in u, v, damage and the bond masks."""
+    wl, nsteps = _small_cases()["config5_long"]
+    out = []
+    for _ in range(2):
+        sim = _sim(wl)
+        assert sim.get_layout()["layout"] == 3
+        sim.step(nsteps)
+        rp, col, intact = sim.get_bond_mask()
+        out.append((sim.get_u().copy(), sim.get_v().copy(), sim.get_damage().copy(), intact.copy()))
+        sim.destroy()
+    assert int((out[0][3] == 0).sum()) > 2 * len(wl.precut), "the case must break bonds"
+    for a, b in zip(out[0], out[1]):
+        assert np.array_equal(a, b)
+
+
 @pytest.mark.parametrize("fracture", [False, True])
 def test_uniform_block_traction_ramp_and_mixed_dofs(fracture):
     """Eq. 2.11 with the ramped body force g(t_n) b and per-dof boundary flags (App. B; C-3, C-4, C-14)
