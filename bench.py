@@ -267,6 +267,10 @@ def measure(name, K, Wm, local, world, want_e2e, want_cpu):
     except Exception:
         pass
     t_dil, t_frc = kd / K * 1e-3, kf / K * 1e-3
+    try:
+        fp64_measured = pd.measure_fp64_rate(5)
+    except Exception:
+        fp64_measured = float("nan")
     dom = ("k_force_update", b_frc, t_frc) if t_frc >= t_dil else ("k_dilatation", b_dil, t_dil)
     achieved = dom[1] / dom[2] / 1e9
     step_s = ms * 1e-3 / K
@@ -295,6 +299,9 @@ def measure(name, K, Wm, local, world, want_e2e, want_cpu):
         "fp64_roofline": {"bound": "alu", "kernel": dom[0], "fp64_per_bond": {"k_dilatation": fp_d, "k_force_update": fp_f},
                           "achieved": (fp_f if dom[0] == "k_force_update" else fp_d) * z / dom[2] / 1e12,
                           "peak": FP64_PEAK / 1e12, "unit": "T FP64 instr/s",
+                          "peak_kind": "derived: 148 SM x 64 FP64 lanes x 1.965 GHz (DESIGN.md 5)",
+                          "peak_measured": fp64_measured / 1e12,
+                          "peak_measured_is": "pd_measure_fp64_rate: 8 independent DFMA chains per thread, 32 warps per SM, best of 5",
                           "frac": (fp_f if dom[0] == "k_force_update" else fp_d) * z / dom[2] / FP64_PEAK,
                           "step_frac": (fp_d + fp_f) * z / step_s / FP64_PEAK},
         "step_roofline": {"algorithmic_bytes_per_step_B2": b_dil + b_frc, "achieved_GBps": (b_dil + b_frc) / step_s / 1e9,

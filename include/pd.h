@@ -217,6 +217,13 @@ PD_API int pd_matrix_step(pd_matrix *pm, int64_t nsteps);
 PD_API int pd_matrix_get(pd_matrix *pm, double *u, double *v, int64_t info[8]);
 PD_API int pd_matrix_destroy(pd_matrix *pm);
 
+/* ---- measured FP64 issue rate of the device (the denominator of the "alu" roofline that bench.py reports beside the HBM
+ * one; DESIGN.md 5 derives the nominal figure 148 SM x 64 lanes x clock) ----
+ * Runs `reps` timed launches of a kernel whose every thread advances 8 independent DFMA chains (32 resident warps per
+ * SM, no memory traffic) and writes the best rate, in FP64 fused multiply-adds per second over all threads, to
+ * *fma_per_s.  stream: cudaStream_t or NULL.  Synchronises.  Errors: PD_ERR_ARG, PD_ERR_ALLOC, PD_ERR_CUDA. */
+PD_API int pd_measure_fp64_rate(int reps, void *stream, double *fma_per_s);
+
 PD_API const char *pd_last_error(void);
 PD_API const char *pd_version(void);
 

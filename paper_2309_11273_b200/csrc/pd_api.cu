@@ -216,6 +216,51 @@ void dev_free_all(pd_sim *s) {
 extern "C" {
 
 const char *pd_last_error(void) { return g_err.c_str(); }
+// 8 independent DFMA chains per thread, 4096 x 8 x 4 fused multiply-adds each
+__global__ void __launch_bounds__(256) k_fp64_rate(double *out, int iters, double a, double b) {
+  double x[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) x[k] = (double)(threadIdx.x + k) * 1e-3;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+#pragma unroll
+      for (int k = 0; k < 8; ++k) x[k] = fma(x[k], a, b);
+  }
+  double sum = 0.0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) sum += x[k];
+  out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = sum;
+}
+
+int pd_measure_fp64_rate(int reps, void *stream, double *fma_per_s) {
+  if (reps <= 0 || !fma_per_s) { pdi::set_error("bad argument"); return PD_ERR_ARG; }
+  int dev = 0, nsm = 0;
+  PD_CUDA(cudaGetDevice(&dev));
+  PD_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+  const cudaStream_t st = (cudaStream_t)stream;
+  const int blocks = nsm * 4, threads = 256, iters = 4096;
+  double *out = nullptr;
+  if (cudaMalloc(&out, sizeof(double) * blocks * threads) != cudaSuccess) { cudaGetLastError(); pdi::set_error("device allocation failed"); return PD_ERR_ALLOC; }
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  double best = 0.0;
+  for (int r = 0; r < reps + 1; ++r) {   // (the first launch is a warm-up)
+    cudaEventRecord(e0, st);
+    k_fp64_rate<<<blocks, threads, 0, st>>>(out, iters, 0.999999, 1e-9);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) break;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (r > 0 && ms > 0.f) best = std::max(best, (double)blocks * threads * iters * 32.0 / (ms * 1e-3));
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(out);
+  PD_CUDA(cudaGetLastError());
+  *fma_per_s = best;
+  return PD_OK;
+}
+
 const char *pd_version(void) {
   return "pd-b200 0.5 (sm_100a, FP64; layouts: uniform lattice [compiled-in 122-offset stencil: mirrored octant walk over "
          "TMA-staged planes; any stencil: table-driven], dense lattice with per-bond geometry, windowed sliced ELL)";

@@ -19,7 +19,7 @@ PD_OK, PD_ERR_ARG, PD_ERR_ISOLATED, PD_ERR_ALLOC, PD_ERR_CUDA, PD_ERR_LIMIT = 0,
 EXPORTS = ["pd_create", "pd_step", "pd_get_u", "pd_get_v", "pd_get_damage", "pd_destroy", "pd_get_stats",
            "pd_get_bond_mask", "pd_get_node_fields", "pd_get_layout", "pd_step_timed", "pd_last_error", "pd_version",
            "pd_matrix_create", "pd_matrix_step", "pd_matrix_get", "pd_matrix_destroy", "pd_adr_step",
-           "pd_gather_u", "pd_scatter_u"]
+           "pd_gather_u", "pd_scatter_u", "pd_measure_fp64_rate"]
 
 
 class PdMaterial(C.Structure):
@@ -82,6 +82,17 @@ def load():
         lib.pd_matrix_destroy.argtypes = [C.c_void_p]
         _lib = lib
     return _lib
+
+
+def measure_fp64_rate(reps: int = 5) -> float:
+    """pd_measure_fp64_rate: FP64 fused multiply-adds per second the device sustains (8 independent chains per thread)."""
+    lib = load()
+    out = C.c_double(0.0)
+    lib.pd_measure_fp64_rate.argtypes = [C.c_int, C.c_void_p, C.POINTER(C.c_double)]
+    rc = lib.pd_measure_fp64_rate(int(reps), None, C.byref(out))
+    if rc != 0:
+        raise PdError(rc, lib.pd_last_error().decode())
+    return float(out.value)
 
 
 def _ptr(a):
