@@ -59,6 +59,7 @@ def byte_model(n, z, dim, fracture):
 # FP64 instructions the arithmetic of the shipped kernels needs per directed bond (dilatation, force), by layout
 # (counted in the SASS of the FAST step: profiles/r02_kernels.md)
 FP64_PER_BOND = {3: (686.0 / 122.0, 1334.0 / 122.0), 2: (7.0, 12.5), 1: (10.0, 22.0), 0: (10.0, 22.0)}
+FP64_PER_BOND_2D = {3: (116.0 / 28.0, 244.0 / 28.0)}   # compiled-in 28-offset stencil: 3 / 5 and 7 / 10 per bond
 
 
 def kernel_source_hash():
@@ -275,6 +276,8 @@ def measure(name, K, Wm, local, world, want_e2e, want_cpu):
     achieved = dom[1] / dom[2] / 1e9
     step_s = ms * 1e-3 / K
     fp_d, fp_f = FP64_PER_BOND.get(lay.get("layout"), (10.0, 22.0))
+    if wl.dim == 2:
+        fp_d, fp_f = FP64_PER_BOND_2D.get(lay.get("layout"), (fp_d, fp_f))
     l2 = 4 * z > 2 * 126e6
     tr = traffic.get(dom[0])
     line = {

@@ -170,7 +170,8 @@ PD_API int pd_get_node_fields(pd_sim *sim, double *m, double *theta);
  * [4]=kernel launches issued by pd_step so far, [5]=bytes of device memory held, [6]=1 if volumes are
  * uniform, [7]=layout: 0 = windowed sliced ELL (any point cloud), 1 = dense lattice, bond geometry per bond
  * (jittered lattices), 2 = dense UNIFORM lattice, bond geometry a constant per stencil offset (the paper's
- * uniform grids), 3 = the same with the 122-offset stencil of horizon 3.015 dx in 3-D compiled in. */
+ * uniform grids), 3 = the same with the stencil of horizon 3.015 dx compiled in (122 offsets in 3-D,
+ * 28 in 2-D). */
 PD_API int pd_get_layout(pd_sim *sim, int64_t counts[8]);
 
 /* measurement aid for the roofline report: like pd_step, but brackets every kernel launch with

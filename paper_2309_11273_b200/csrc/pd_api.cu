@@ -262,7 +262,7 @@ int pd_measure_fp64_rate(int reps, void *stream, double *fma_per_s) {
 }
 
 const char *pd_version(void) {
-  return "pd-b200 0.5 (sm_100a, FP64; layouts: uniform lattice [compiled-in 122-offset stencil: mirrored octant walk over "
+  return "pd-b200 0.6 (sm_100a, FP64; layouts: uniform lattice [compiled-in 122-offset (3-D) and 28-offset (2-D) stencils over "
          "TMA-staged planes; any stencil: table-driven], dense lattice with per-bond geometry, windowed sliced ELL)";
 }
 
@@ -579,7 +579,7 @@ int pd_get_layout(pd_sim *s, int64_t counts[8]) {
   if (!s || !counts) { pdi::set_error("null argument"); return PD_ERR_ARG; }
   counts[0] = s->n; counts[1] = s->npad; counts[2] = s->Z; counts[3] = s->nentries * 32;
   counts[4] = s->launches; counts[5] = (int64_t)s->bytes_held; counts[6] = s->uniform_v ? 1 : 0;
-  counts[7] = s->lat.on ? (s->lat.uniform ? (pdi::ball_eligible(s) ? 3 : 2) : 1) : 0;
+  counts[7] = s->lat.on ? (s->lat.uniform ? (pdi::ball_eligible(s) || pdi::disc_eligible(s) ? 3 : 2) : 1) : 0;
   return PD_OK;
 }
 

@@ -133,8 +133,8 @@ struct PdLattice {
   int32_t *off2bit = nullptr;      // [(2S2+1)(2S1+1)(2S0+1)] offset -> bit index or -1
   double r2lb[128];                // per stencil bit: min over all bonds of ||xi||^2 exactly as the step kernels
                                    // compute it (break-test filter: dot < s_c * r2lb  =>  the bond cannot break)
-  void *cache[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // host: prepared launch arguments of the step
-                                   // kernels ([0], [1]: pd_lattice_uniform.cu; [2], [3]: pd_lattice_step.cu; [4], [5]: pd_lattice_ball.cu)
+  void *cache[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // host: prepared launch arguments of the step
+                                   // kernels ([0], [1]: pd_lattice_uniform.cu; [2], [3]: pd_lattice_step.cu; [4], [5]: pd_lattice_ball.cu; [6], [7]: pd_lattice_disc.cu)
   // pd_lattice_ball.cu: octant words of mask / nofail [8][npad] and the exact-pass tables (device)
   uint32_t *mask8 = nullptr, *nf8 = nullptr;
   void *ball_q8 = nullptr, *ball_wl = nullptr;   // table of the octant copies; worklist of the break test
@@ -216,11 +216,16 @@ void lat_free_cache(pd_sim *s);
 int ulat_launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
 int ulat_launch_force_update(pd_sim *s);
 void ulat_free_cache(pd_sim *s);
-// pd_lattice_ball.cu: return 1 if launched, 0 if the lattice's stencil is not the compiled-in ball
+// pd_lattice_ball.cu: return 1 if launched, 0 if the lattice's stencil is not the compiled-in ball, < 0 on error
 int ball_launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
 int ball_launch_force_update(pd_sim *s);
 void ball_free_cache(pd_sim *s);
 bool ball_eligible(const pd_sim *s);
+// pd_lattice_disc.cu: the same for the 2-D 28-offset stencil
+int disc_launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
+int disc_launch_force_update(pd_sim *s);
+void disc_free_cache(pd_sim *s);
+bool disc_eligible(const pd_sim *s);
 // pd_step.cu
 int launch_dilatation(pd_sim *s, double *theta_out, bool do_break);
 int launch_force_update(pd_sim *s);

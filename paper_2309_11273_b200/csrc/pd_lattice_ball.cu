@@ -825,13 +825,13 @@ BPrepared *ball_prepare(pd_sim *s, bool force) {
         memcpy(&bits, &thr, 8);
         a.thr_hi[i * i + j * j + k * k] = std::min(a.thr_hi[i * i + j * j + k * k], (int)(bits >> 32));
       }
-  if (!ball_tables(s)) return pp;
+  if (!ball_tables(s)) { slot = nullptr; delete pp; return nullptr; }   // device allocation failed: nothing cached
   a.q8 = (const int2 *)l.ball_q8;
   a.mask8 = l.mask8; a.nf8 = l.nf8;
   if (!l.ball_tfull) {   // the warp-tile flags (kept in step by the exact pass)
     const int ntiles = ((l.PZ + BRZ - 1) / BRZ) * l.PY * a.nxc;
     uint8_t *tf = (uint8_t *)pdi::dev_alloc(s, (size_t)ntiles);
-    if (!tf) return pp;
+    if (!tf) { slot = nullptr; delete pp; return nullptr; }
     a.tfull = tf;
     k_ball_tileflags<BRZ><<<(unsigned)(((int64_t)ntiles * 32 + 255) / 256), 256, 0, s->stream>>>(a, ntiles);
     if (cudaGetLastError() != cudaSuccess || cudaStreamSynchronize(s->stream) != cudaSuccess) { cudaGetLastError(); return pp; }
@@ -842,7 +842,7 @@ BPrepared *ball_prepare(pd_sim *s, bool force) {
     const size_t ntiles = (size_t)((l.PZ + BRZ - 1) / BRZ) * l.PY * a.nxc;
     void *wl = pdi::dev_alloc(s, ntiles * 32 * sizeof(BEntry<BRZ>));
     int *cnt = (int *)pdi::dev_alloc(s, sizeof(int));
-    if (!wl || !cnt) return pp;
+    if (!wl || !cnt) { slot = nullptr; delete pp; return nullptr; }
     l.ball_wl = wl; l.ball_wl_count = cnt;
   }
   a.wl = l.ball_wl; a.wl_count = l.ball_wl_count;
@@ -873,9 +873,10 @@ void ball_free_cache(pd_sim *s) {
   }
 }
 
-// 1: launched; 0: the lattice is not the ball (the caller takes the table-driven kernels)
+// 1: launched; 0: the lattice is not the ball (the caller takes the table-driven kernels); < 0: error
 int ball_launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
   BPrepared *pp = ball_prepare(s, false);
+  if (!pp) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
   if (!pp->ok) return 0;
   const PdLattice &l = s->lat;
   BArgs &a = pp->a;
@@ -895,6 +896,7 @@ int ball_launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
 
 int ball_launch_force_update(pd_sim *s) {
   BPrepared *pp = ball_prepare(s, true);
+  if (!pp) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
   if (!pp->ok) return 0;
   const PdLattice &l = s->lat;
   BArgs &a = pp->a;

@@ -672,6 +672,7 @@ namespace pdi {
 
 void ulat_free_cache(pd_sim *s) {
   ball_free_cache(s);
+  disc_free_cache(s);
   for (int q = 0; q < 2; ++q) {
     delete (UPrepared *)s->lat.cache[q];
     s->lat.cache[q] = nullptr;
@@ -679,7 +680,8 @@ void ulat_free_cache(pd_sim *s) {
 }
 
 int ulat_launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
-  if (ball_launch_dilatation(s, theta_out, do_break)) return PD_OK;   // the compiled-in 122-offset stencil
+  if (int rc = ball_launch_dilatation(s, theta_out, do_break)) return rc > 0 ? PD_OK : rc;   // the compiled-in 122-offset stencil (3-D)
+  if (int rc = disc_launch_dilatation(s, theta_out, do_break)) return rc > 0 ? PD_OK : rc;   // the compiled-in 28-offset stencil (2-D)
   UPrepared *pp = ulat_prepare(s, false);
   if (!pp) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
   const PdLattice &l = s->lat;
@@ -694,7 +696,8 @@ int ulat_launch_dilatation(pd_sim *s, double *theta_out, bool do_break) {
 }
 
 int ulat_launch_force_update(pd_sim *s) {
-  if (ball_launch_force_update(s)) return PD_OK;
+  if (int rc = ball_launch_force_update(s)) return rc > 0 ? PD_OK : rc;
+  if (int rc = disc_launch_force_update(s)) return rc > 0 ? PD_OK : rc;
   UPrepared *pp = ulat_prepare(s, true);
   if (!pp) { set_error("device allocation failed"); return PD_ERR_ALLOC; }
   const PdLattice &l = s->lat;

@@ -14,21 +14,22 @@ TOL = 1e-10
 
 # the code paths of the library: the layout is chosen inside pd_create; the environment
 # switches exist for exactly this purpose (and for profiling).  Layout codes (pd_get_layout): 3 = uniform lattice with
-# the compiled-in 122-offset stencil (3-D, horizon 3.015 dx: config 5), 2 = uniform
-# lattice (constant bond geometry per stencil offset; the default on the unjittered grids of configs 1, 2, 3),
+# the stencil of horizon 3.015 dx compiled in (122 offsets in 3-D, 28 in 2-D: configs 1, 2, 3, 5), 2 = uniform
+# lattice (constant bond geometry per stencil offset, table-driven kernels: any other stencil),
 # 1 = dense lattice with per-bond geometry (jittered config 4; PD_LAT_UNIFORM=0 forces it), 0 = sliced ELL.
 LAYOUTS = {
     "default": ({}, None),
     # uniform lattice, records through L1 instead of TMA-staged planes; rows per lane swapped (2 in 3-D, 4 in 2-D);
     # plain launches instead of CUDA graphs
-    # (PD_BALL=0: the table-driven kernels also where the stencil is the compiled-in 122-offset ball of pd_lattice_ball.cu)
+    # (PD_BALL=0, PD_DISC=0: the table-driven kernels also where the stencil is the compiled-in 122-offset ball of
+    # pd_lattice_ball.cu / the 28-offset disc of pd_lattice_disc.cu)
     "uniform_direct": ({"PD_ULAT_STAGED": "0", "PD_ULAT_DIL_ROWS": "-1", "PD_ULAT_FRC_ROWS": "-1", "PD_GRAPH": "0",
-                        "PD_BALL": "0"}, None),
+                        "PD_BALL": "0", "PD_DISC": "0"}, None),
     # staged planes with 3 buffers in flight, rows per lane swapped, 2 row groups per CTA
     "uniform_nb3": ({"PD_ULAT_NB": "3", "PD_ULAT_DIL_ROWS": "-1", "PD_ULAT_FRC_ROWS": "-1", "PD_ULAT_DIL_CY": "2",
-                     "PD_ULAT_FRC_CY": "2", "PD_BALL": "0"}, None),
+                     "PD_ULAT_FRC_CY": "2", "PD_BALL": "0", "PD_DISC": "0"}, None),
     # table-driven staged kernels with their default shape
-    "uniform_table": ({"PD_BALL": "0"}, None),
+    "uniform_table": ({"PD_BALL": "0", "PD_DISC": "0"}, None),
     # compiled-in stencil kernels in their other launch shape: 4 rows per CTA, 3 plane buffers in flight
     "ball_cy4_nb3": ({"PD_BALL_CY": "4", "PD_BALL_NB": "3"}, None),
     "lattice_general": ({"PD_LAT_UNIFORM": "0"}, 1),
@@ -36,7 +37,7 @@ LAYOUTS = {
     "sliced_ell": ({"PD_FORCE_GENERIC": "1"}, 0),
 }
 _ENV_KEYS = ("PD_LAT_UNIFORM", "PD_FORCE_GENERIC", "PD_DIR_DIL_ROWS", "PD_DIR_FRC_ROWS", "PD_ULAT_DIL_ROWS",
-             "PD_ULAT_FRC_ROWS", "PD_ULAT_STAGED", "PD_ULAT_NB", "PD_ULAT_DIL_CY", "PD_ULAT_FRC_CY", "PD_GRAPH", "PD_BALL", "PD_BALL_CY", "PD_BALL_NB")
+             "PD_ULAT_FRC_ROWS", "PD_ULAT_STAGED", "PD_ULAT_NB", "PD_ULAT_DIL_CY", "PD_ULAT_FRC_CY", "PD_GRAPH", "PD_BALL", "PD_BALL_CY", "PD_BALL_NB", "PD_DISC")
 
 
 @pytest.fixture(params=list(LAYOUTS))
@@ -56,7 +57,8 @@ def _expect_layout(code, wl):
     if wl.name == "block3d" and wl.meta.get("jitter", 1.0) != 0.0:
         return 1
     import os
-    return 3 if wl.dim == 3 and os.environ.get("PD_BALL", "1") != "0" else 2   # 3: the compiled-in 122-offset stencil
+    # 3: the kernels with the stencil compiled in (122 offsets in 3-D, 28 in 2-D)
+    return 3 if os.environ.get("PD_BALL" if wl.dim == 3 else "PD_DISC", "1") != "0" else 2
 
 
 def _oracle(wl):
@@ -284,11 +286,18 @@ def test_threshold_bond(layout):
         sim.destroy()
 
 
-def test_step_error_is_returned_and_state_kept():
+@pytest.mark.parametrize("case", ["cylinder3d", "branching2d_table"])
+def test_step_error_is_returned_and_state_kept(case, monkeypatch):
     """a launch that cannot be prepared (device allocation failing inside pd_step) must come back as an error
-    code and leave the step counter and the buffers where they were"""
+    code and leave the step counter and the buffers where they were.  (The compiled-in 3-D stencil kernels allocate
+    their octant words, tile flags and worklist at the first step, the table-driven kernels their tables; the
+    compiled-in 2-D kernels allocate nothing, hence PD_DISC=0 for the 2-D case.)"""
     from paper_2309_11273_b200 import pd, workloads as W
-    wl = W.branching2d(nx=40, ny=24)
+    if case == "cylinder3d":
+        wl = W.cylinder3d(r_cells=9, l_cells=34, omega=400.0)
+    else:
+        monkeypatch.setenv("PD_DISC", "0")
+        wl = W.branching2d(nx=40, ny=24)
     o = _oracle(wl)
     sim = _sim(wl)
     sim._rt.fail_allocs = True          # fault injection: the allocator callback returns NULL
