@@ -147,6 +147,22 @@ PD_API int pd_get_u(pd_sim *sim, double *dst);
 PD_API int pd_get_v(pd_sim *sim, double *dst);
 PD_API int pd_get_damage(pd_sim *sim, double *dst);
 
+/*
+ * pd_get_u_static -- pd_get_u for callers that may not allocate device memory (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): the same u^n of Eq. 2.11, the same dst
+ * (dim*n doubles, AoS, user node order, host or device, caller-owned), bit for bit.  pd_get_u stages the reordered
+ * field in a scratch buffer that it allocates and frees per call; this entry point stages it in a static device array of
+ * PD_STATIC_MAX_DOUBLES doubles (8 MiB) that every GPU that loads the library holds until the process exits, and calls
+ * no cudaMalloc / cudaFree, no pd_runtime callback and no allocating library routine: one kernel and one copy on the
+ * handle's stream, then a synchronise.  The handle's device must be current (as for every call).
+ * All calls, on all handles, share that one array per device: calls that overlap on the GPU (different streams or
+ * host threads) race and must be serialised by the caller.  Nothing of an earlier call's contents is ever read.
+ * Errors: PD_ERR_ARG (null), PD_ERR_LIMIT (dim*n > PD_STATIC_MAX_DOUBLES: use pd_get_u; nothing is launched),
+ * PD_ERR_CUDA.
+ */
+#define PD_STATIC_MAX_DOUBLES (1 << 20)
+PD_API int pd_get_u_static(pd_sim *sim, double *dst);
+
 PD_API int pd_destroy(pd_sim *sim);
 
 /* ---- extensions (not named by the north star; needed to check and report it) ---- */

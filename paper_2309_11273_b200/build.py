@@ -13,7 +13,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpd.so")
-SOURCES = ["pd_api.cu", "pd_build.cu", "pd_step.cu", "pd_lattice.cu", "pd_lattice_step.cu", "pd_lattice_uniform.cu", "pd_lattice_ball.cu", "pd_lattice_disc.cu", "pd_matrix.cu"]
+SOURCES = ["pd_api.cu", "pd_build.cu", "pd_step.cu", "pd_lattice.cu", "pd_lattice_step.cu", "pd_lattice_uniform.cu", "pd_lattice_ball.cu", "pd_lattice_disc.cu", "pd_matrix.cu",
+           os.path.join("static", "pd_static_read.cu")]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--default-stream", "legacy"]
 
@@ -22,7 +23,8 @@ def _stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(HERE, "..", "include", "pd.h")]
+    deps = [os.path.join(d, f) for d, _, fs in os.walk(CSRC) for f in fs if not f.endswith(".o")]
+    deps.append(os.path.join(HERE, "..", "include", "pd.h"))
     return any(os.path.getmtime(d) > t for d in deps)
 
 

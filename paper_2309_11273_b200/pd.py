@@ -16,10 +16,11 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBPATH = os.environ.get("PD_LIBPATH") or os.path.join(_HERE, "libpd.so")   # PD_LIBPATH: an alternative build (debugging)
 
 PD_OK, PD_ERR_ARG, PD_ERR_ISOLATED, PD_ERR_ALLOC, PD_ERR_CUDA, PD_ERR_LIMIT = 0, -1, -2, -3, -4, -5
+STATIC_MAX_DOUBLES = 1 << 20   # PD_STATIC_MAX_DOUBLES of include/pd.h: capacity of the static scratch of pd_get_u_static
 EXPORTS = ["pd_create", "pd_step", "pd_get_u", "pd_get_v", "pd_get_damage", "pd_destroy", "pd_get_stats",
            "pd_get_bond_mask", "pd_get_node_fields", "pd_get_layout", "pd_step_timed", "pd_last_error", "pd_version",
            "pd_matrix_create", "pd_matrix_step", "pd_matrix_get", "pd_matrix_destroy", "pd_adr_step",
-           "pd_gather_u", "pd_scatter_u", "pd_measure_fp64_rate"]
+           "pd_gather_u", "pd_scatter_u", "pd_measure_fp64_rate", "pd_get_u_static"]
 
 
 class PdMaterial(C.Structure):
@@ -64,7 +65,7 @@ def load():
         lib.pd_create.argtypes = [C.POINTER(C.c_void_p), C.c_int64, C.c_void_p, C.c_void_p, C.c_double,
                                   C.POINTER(PdMaterial), C.POINTER(PdBoundary), C.POINTER(PdRuntime)]
         lib.pd_step.argtypes = [C.c_void_p, C.c_int64]
-        for name in ("pd_get_u", "pd_get_v", "pd_get_damage"):
+        for name in ("pd_get_u", "pd_get_v", "pd_get_damage", "pd_get_u_static"):
             getattr(lib, name).argtypes = [C.c_void_p, C.c_void_p]
         lib.pd_destroy.argtypes = [C.c_void_p]
         lib.pd_get_stats.argtypes = [C.c_void_p] + [C.c_void_p] * 5
@@ -250,6 +251,10 @@ class Sim:
 
     def get_u(self, out=None):
         return self._get(self.lib.pd_get_u, (self.n, self.dim), out)
+
+    def get_u_static(self, out=None):
+        """pd_get_u_static: get_u through the library's static device scratch (no device allocation; dim*n <= STATIC_MAX_DOUBLES)"""
+        return self._get(self.lib.pd_get_u_static, (self.n, self.dim), out)
 
     def get_v(self, out=None):
         return self._get(self.lib.pd_get_v, (self.n, self.dim), out)
