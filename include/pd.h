@@ -241,6 +241,16 @@ PD_API int pd_matrix_destroy(pd_matrix *pm);
  * *fma_per_s.  stream: cudaStream_t or NULL.  Synchronises.  Errors: PD_ERR_ARG, PD_ERR_ALLOC, PD_ERR_CUDA. */
 PD_API int pd_measure_fp64_rate(int reps, void *stream, double *fma_per_s);
 
+/* ---- measured issue rates behind DESIGN.md 5.1 "why every directed bond is evaluated from both ends" ----
+ * t_ij = t_ji in Eq. 2.2: one end of a bond could compute the term and hand it to the other end, over
+ * the lanes of a warp by a shuffle or between warps through shared memory.  Times four kernels at the launch shape of
+ * pd_measure_fp64_rate and writes, over all threads, per second:
+ *   per_s[0] FP64 fused multiply-adds alone; per_s[1] 64-bit lane shifts alone (2 SHFL.32 each); per_s[2] groups of
+ *   {1 lane-shifted double + 5 dependent DFMA} (the trade of the force pass); per_s[3] doubles through shared memory
+ *   (8-byte store + load of another lane's slot).
+ * stream: cudaStream_t or NULL.  Allocates nothing.  Synchronises.  Errors: PD_ERR_ARG, PD_ERR_CUDA. */
+PD_API int pd_measure_pair_exchange(int reps, void *stream, double per_s[4]);
+
 PD_API const char *pd_last_error(void);
 PD_API const char *pd_version(void);
 

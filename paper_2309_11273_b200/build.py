@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpd.so")
 SOURCES = ["pd_api.cu", "pd_build.cu", "pd_step.cu", "pd_lattice.cu", "pd_lattice_step.cu", "pd_lattice_uniform.cu", "pd_lattice_ball.cu", "pd_lattice_disc.cu", "pd_matrix.cu",
-           os.path.join("static", "pd_static_read.cu")]
+           os.path.join("aux", "pd_static_read.cu"), os.path.join("aux", "pd_probe.cu")]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--default-stream", "legacy"]
 

@@ -20,7 +20,8 @@ STATIC_MAX_DOUBLES = 1 << 20   # PD_STATIC_MAX_DOUBLES of include/pd.h: capacity
 EXPORTS = ["pd_create", "pd_step", "pd_get_u", "pd_get_v", "pd_get_damage", "pd_destroy", "pd_get_stats",
            "pd_get_bond_mask", "pd_get_node_fields", "pd_get_layout", "pd_step_timed", "pd_last_error", "pd_version",
            "pd_matrix_create", "pd_matrix_step", "pd_matrix_get", "pd_matrix_destroy", "pd_adr_step",
-           "pd_gather_u", "pd_scatter_u", "pd_measure_fp64_rate", "pd_get_u_static"]
+           "pd_gather_u", "pd_scatter_u", "pd_measure_fp64_rate", "pd_get_u_static",
+           "pd_measure_pair_exchange"]
 
 
 class PdMaterial(C.Structure):
@@ -94,6 +95,18 @@ def measure_fp64_rate(reps: int = 5) -> float:
     if rc != 0:
         raise PdError(rc, lib.pd_last_error().decode())
     return float(out.value)
+
+
+def measure_pair_exchange(reps: int = 5) -> dict:
+    """pd_measure_pair_exchange: issue rates (per second, all threads) of FP64 FMAs, 64-bit lane shifts, groups of one lane
+    shift + 5 dependent FMAs, and doubles through shared memory"""
+    lib = load()
+    out = (C.c_double * 4)()
+    lib.pd_measure_pair_exchange.argtypes = [C.c_int, C.c_void_p, C.c_void_p]
+    rc = lib.pd_measure_pair_exchange(int(reps), None, C.addressof(out))
+    if rc != 0:
+        raise PdError(rc, lib.pd_last_error().decode())
+    return dict(zip(("dfma_per_s", "shift64_per_s", "shift64_plus_5dfma_per_s", "smem_double_per_s"), map(float, out)))
 
 
 def _ptr(a):

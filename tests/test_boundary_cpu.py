@@ -18,7 +18,7 @@ def test_library_builds_loads_and_exports_header_symbols():
     build.build()
     lib = pd.load()
     names = declared_symbols()
-    assert len(names) == 22 and set(names) == set(pd.EXPORTS)
+    assert len(names) == 23 and set(names) == set(pd.EXPORTS)
     for name in names:
         assert getattr(lib, name) is not None
     assert b"sm_100a" in lib.pd_version()
