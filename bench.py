@@ -63,7 +63,9 @@ FP64_PER_BOND_2D = {3: (116.0 / 28.0, 244.0 / 28.0)}   # compiled-in 28-offset s
 
 
 def kernel_source_hash():
-    """sha256 over the CUDA sources: ncu traffic figures are only quoted for the build they were captured on"""
+    """sha256 over the CUDA sources of the step path (csrc/*.cu, *.cuh): ncu traffic figures are only quoted for the
+    build they were captured on.  csrc/aux/ (read-back through static scratch, issue-rate probes) holds separately
+    compiled translation units that no step kernel includes or calls and is not part of it."""
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2309_11273_b200", "csrc")
     for f in sorted(os.listdir(d)):
@@ -163,7 +165,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": "node-steps/s", "n_gpus": args.gpus,
         "steps": per_step, "warmup": 1, "ms_per_step": 1e3 * dt / per_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": name, "sample": desc, "nodes": wl.n, "directed_bonds": z},
+        "config": {"workload": f"{name}:{wl.name}", "sample": desc, "nodes": wl.n, "directed_bonds": z},
         "bond_updates_per_s": z * per_step / dt,
         "cpu_baseline": {"value": val, "unit": "node-steps/s", "cores": cores, "kind": "oracle",
                          "sample": f"{desc}, {per_step} steps"},
