@@ -8,9 +8,10 @@ counts"), in the launch configuration bench.py times (default layout, CUDA graph
 
 Config 5 at omega = 100 rad/s starts breaking bonds between steps 500 and 1000 and has 18.2 M directed bonds
 broken after its 2000 steps (bench.py times exactly that run and prints the counts); the oracle needs about 20
-minutes for those 6.3e9 node-steps, so the full-size fracture parity is taken on config 5' with omega raised to
-400 rad/s (bonds break from step 3 on, 11.8 M directed bonds broken after 300 steps), as the small test does.
-The 2000-step run of config 5' at omega = 100 against the oracle is recorded in profiles/r02_parity_full.md.
+minutes for those 6.3e9 node-steps, so inside this suite the full-size fracture parity is taken on config 5' with
+omega raised to 400 rad/s (bonds break from step 3 on, 11.8 M directed bonds broken after 300 steps), as the small
+test does.  The 2000-step run of config 5 itself against the oracle (tests/run_full_parity.py: identical broken sets
+at steps 500, 1000, 1500 and 2000) is recorded in profiles/r02_parity_full.md.
 Bonds within 1e-9 relative of s_c at their breaking step are counted by the oracle (near_total) and reported.
 """
 import time
